@@ -122,11 +122,27 @@ static ld adapt_rec(orc_fn f, const void* ctx, ld a, ld b, ld whole, ld tol, int
     return adapt_rec(f, ctx, a, m, L, tol, depth + 1) + adapt_rec(f, ctx, m, b, R, tol, depth + 1);
 }
 
-static ld integrate(orc_fn f, const void* ctx, ld a, ld b)
+static ld integrate_panel(orc_fn f, const void* ctx, ld a, ld b)
 {
     ld whole = gl_panel(f, ctx, a, b);
     ld tol = 1e-17L * fabsl(whole) + 1e-300L;
     return adapt_rec(f, ctx, a, b, whole, tol, 0);
+}
+
+/* Integral over [0,1] of an integrand that has a boundary layer of width `layer` at x = 0
+ * (the Eq 32/35 integrands vary on the scale x ~ cos(alpha)/sqrt(q(0)) there).  The interval is
+ * first cut at x = 1/2, 1/4, ... down to `layer`, and every piece is integrated adaptively:
+ * a single top-level panel cannot see a layer narrower than its first node and would accept
+ * the layer-free value (an O(cos alpha) error for |alpha - pi/2| < ~1e-8). */
+static ld integrate01(orc_fn f, const void* ctx, ld layer)
+{
+    ld sum = 0.0L, hi = 1.0L;
+    for (int j = 0; j < 70 && hi > layer; ++j) {
+        ld lo = 0.5L * hi;
+        sum += integrate_panel(f, ctx, lo, hi);
+        hi = lo;
+    }
+    return sum + integrate_panel(f, ctx, 0.0L, hi);
 }
 
 /* ------------------------------------------------------------------------------------
@@ -135,7 +151,7 @@ static ld integrate(orc_fn f, const void* ctx, ld a, ld b)
  *   psi(u,alpha) = 2 sin(alpha)/sqrt(1-u) * Int_0^1 x dx / sqrt(cos^2 alpha + x^2 q)
  *   q = [2 - x^2 - u (1-x^2)^2/(1-u)] sin^2 alpha                                (alpha <= pi/2)
  * ---------------------------------------------------------------------------------- */
-typedef struct { ld u, sa2, ca2; } bend_ctx;
+typedef struct { ld u, sa2, ca2, layer; } bend_ctx;
 
 static inline ld q_of_x(ld x, const bend_ctx* c)
 {
@@ -168,22 +184,25 @@ static void bend_ctx_set(bend_ctx* c, ld u, ld alpha)
 {
     ld sa = sinl(alpha), ca = cosl(alpha);
     c->u = u; c->sa2 = sa * sa; c->ca2 = ca * ca;
+    /* width of the x -> 0 layer of D = cos^2 a + x^2 q:  |cos a| / sqrt(q(0)),  q(0) = (2 - u/(1-u)) sin^2 a */
+    ld q0 = (2.0L - u / (1.0L - u)) * c->sa2;
+    c->layer = (q0 > 0.0L) ? fabsl(ca) / sqrtl(q0) : 1.0L;
 }
 
 static ld psi_out(ld u, ld alpha)          /* 0 <= alpha <= pi/2 */
 {
     bend_ctx c; bend_ctx_set(&c, u, alpha);
-    return 2.0L * sinl(alpha) / sqrtl(1.0L - u) * integrate(f_psi, &c, 0.0L, 1.0L);
+    return 2.0L * sinl(alpha) / sqrtl(1.0L - u) * integrate01(f_psi, &c, c.layer);
 }
 static ld dpsi_out_analytic(ld u, ld alpha) /* 0 <= alpha < pi/2 */
 {
     bend_ctx c; bend_ctx_set(&c, u, alpha);
-    return 2.0L * cosl(alpha) / sqrtl(1.0L - u) * integrate(f_dpsi, &c, 0.0L, 1.0L);
+    return 2.0L * cosl(alpha) / sqrtl(1.0L - u) * integrate01(f_dpsi, &c, c.layer);
 }
 static ld lag_out(ld u, ld alpha)          /* G(u,alpha) = c dt_p / R, 0 <= alpha <= pi/2 */
 {
     bend_ctx c; bend_ctx_set(&c, u, alpha);
-    return 2.0L * c.sa2 / (1.0L - u) * integrate(f_lag, &c, 0.0L, 1.0L);
+    return 2.0L * c.sa2 / (1.0L - u) * integrate01(f_lag, &c, c.layer);
 }
 
 /* periastron ratio rho = R_p / R for an inward ray, Eq 14 */

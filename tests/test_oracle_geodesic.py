@@ -165,3 +165,17 @@ def test_alpha_of_psi_inverts_psi():
         a2 = o.alpha_of_psi(u, ps, np.pi / 2 + 0.1)
         assert abs(a2 - a) < 1e-13
     assert o.alpha_of_psi(U0, 3.0, np.pi / 2) is None
+
+
+@pytest.mark.parametrize("eps", [1e-6, 1e-8, 1e-9, 1e-10, 1e-11])
+def test_p5_no_missed_boundary_layer_next_to_the_limb(eps):
+    """psi and the lag are smooth in alpha through pi/2 (pin P5: one-sided slopes 1.67572 / 1.67583 and
+    2.06989 / 2.07004 at h = 1e-4), so the secant slope over ANY small step must sit between
+    them.  The Eq 32/35 integrands have a layer of width ~cos(alpha) at x = 0; a quadrature that does not
+    resolve it returns psi(pi/2 - eps) = psi(pi/2) for eps < ~1e-8 (slope 0)."""
+    hp = np.pi / 2
+    s_psi = (o.psi(U0, hp) - o.psi(U0, hp - eps)) / eps
+    s_lag = (o.lag(U0, hp) - o.lag(U0, hp - eps)) / eps
+    tol = 3e-4 + 1e-15 / eps          # probe spread + double rounding of the difference
+    assert abs(s_psi - 1.675775) < tol
+    assert abs(s_lag - 2.069965) < tol
