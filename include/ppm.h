@@ -1,0 +1,153 @@
+/*
+ * ppm.h -- C ABI of the B200-native pulse-profile-modeling (PPM) hot path.
+ *
+ * One likelihood-call evaluation of the energy-resolved pulse profile of a rotating neutron
+ * star in the oblate-Schwarzschild + Doppler (OS+D) picture of arxiv/paper_2510_07764
+ * (Zhou & Huang).  Citations are "PAPER.md:<line>" plus the section / equation; readings
+ * R0..R22 of the places where the paper is silent or garbled are listed in DESIGN.md.
+ *
+ * Everything behind this boundary is hand-written CUDA for sm_100a.  There is NO CPU
+ * fallback: every entry point fails with PPM_ERR_CUDA when no device is usable.
+ *
+ * Conventions
+ *   - "dev" pointers are CUDA device pointers on the context's device; "host" pointers are
+ *     ordinary host memory.  The caller owns every buffer it passes; the context copies the
+ *     tables given to ppm_create / ppm_load_atmosphere / ppm_set_response and owns only its
+ *     own scratch.  Outputs are fully overwritten.
+ *   - All work is enqueued on the cudaStream_t given to ppm_create (pass
+ *     torch.cuda.current_stream().cuda_stream, or NULL for the default stream).  Calls that
+ *     take only device pointers are asynchronous and never synchronise; ppm_create,
+ *     ppm_load_atmosphere, ppm_set_response, ppm_*_host and ppm_debug_* synchronise the stream.
+ *   - One context per stream; a context is not thread-safe.
+ *   - Return value: 0 on success, a negative PPM_ERR_* otherwise; ppm_last_error() gives text.
+ *   - Per-vector physics failures do not fail the call: status[b] carries the bits below,
+ *     that vector's flux is NaN and its log-likelihood -inf.
+ *
+ * Parameter vector (P = 8 + 8*n_spots doubles, row-major [B][P]; "(M, R, nu), i,
+ * the hotspot's shape, position, and size"; D of Eq 21; N_H PAPER.md:270):
+ *   [0] M / M_sun   [1] R_eq / km   [2] nu / Hz (seen at infinity)   [3] cos i
+ *   [4] D / kpc     [5] N_H / 1e20 cm^-2   [6] phase offset / cycles   [7] reserved
+ *   per spot s (offset 8+8s): [0] theta_c  [1] phi_c  [2] zeta (angular radius, rad)
+ *   [3] log10 T_eff/K  [4] theta_m  [5] phi_m  [6] zeta_m (0 => no omitted region)  [7] reserved
+ */
+#ifndef PPM_H_
+#define PPM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PPM_OK            0
+#define PPM_ERR_ARG      -1   /* invalid argument / shape */
+#define PPM_ERR_NOMEM    -2   /* host or device allocation failed */
+#define PPM_ERR_CUDA     -3   /* CUDA runtime error (incl. no usable device) */
+#define PPM_ERR_STATE    -4   /* wrong state, e.g. table emission without a loaded atmosphere */
+#define PPM_ERR_BATCH    -5   /* B > max_batch */
+
+#define PPM_STATUS_COMPACTNESS 1  /* R_S/R outside (0, 0.56] (reading R4) */
+#define PPM_STATUS_INPUT       2  /* non-finite input, beta_eq >= 1, bad M/R/D/cos i */
+#define PPM_STATUS_SPOT        4  /* invalid spot (zeta <= 0, angles outside [0, pi]) */
+
+#define PPM_EMISSION_BLACKBODY   0  /* isotropic blackbody, Eq C.5 */
+#define PPM_EMISSION_TABLE_CUBIC 1  /* 4-D table, cubic Lagrange on all axes (strategy a) */
+#define PPM_EMISSION_TABLE_MIXED 2  /* 4-D table, mixed order (strategy d) */
+
+#define PPM_MAX_SPOTS 4
+
+typedef struct ppm_ctx ppm_ctx; /* opaque: device tables, scratch, a copy of the energy grid */
+
+typedef struct {
+    int32_t n_spots;    /* 1..PPM_MAX_SPOTS emitting components (overlaps add, reading R18) */
+    int32_t n_theta;    /* colatitude rows of each spot's bounding-box grid (reading R1) */
+    int32_t n_phi;      /* azimuth cells per row of that grid */
+    int32_t n_phase;    /* output phases, phi_out[k] = k / n_phase (reading R3) */
+    int32_t n_fp;       /* fine template phases N_fp (Table 4); 0 -> max(192, 2*n_phase) */
+    int32_t n_energy;   /* observed photon energies (keV), given to ppm_create */
+    int32_t emission;   /* PPM_EMISSION_* */
+    int32_t precision;  /* 0 = fp64 everywhere (the only mode implemented) */
+    int32_t oblate;     /* 0 spherical S+D (o2 = 0, g = g0); 1 oblate OS+D (Eq 7-11) */
+    int32_t max_batch;  /* largest B accepted by ppm_evaluate / ppm_fold_response / ppm_loglike */
+    int32_t device;     /* CUDA ordinal */
+} ppm_config;
+
+/* Create a context: copies the energy grid (host, [n_energy], keV, strictly increasing),
+ * allocates scratch, builds the quadrature rule used by the lookup-build kernel.
+ * cuda_stream is a cudaStream_t (may be NULL).  *out receives the context. */
+int ppm_create(const ppm_config* cfg, const double* energies_keV, void* cuda_stream, ppm_ctx** out);
+int ppm_destroy(ppm_ctx* ctx);
+
+/* Load the 4-D atmosphere table log10(I / T_eff^3)[logT][logg][mu][logx], C order, x = E/kT
+ * (base-10 logs, reading R13a).  Axes: host, strictly increasing, >= 4 nodes
+ * each; logx must be uniformly spaced (as the paper's 166-point -1.3..2.0 axis is).
+ * values: host pointer, or device pointer when values_on_device != 0.  Everything is copied. */
+int ppm_load_atmosphere(ppm_ctx* ctx, const double* logT, int nT, const double* logg, int ng,
+                        const double* mu, int nmu, const double* logx, int nx,
+                        const double* values, int values_on_device);
+
+/* Set the banded response (Eq 52-55; reading R15) and the ISM optical depth
+ * per 1e20 cm^-2 (Eq 22/51; reading R16).  Row e of rsp_band covers
+ * channels first_chan[e] .. first_chan[e]+band_w-1 (entries outside [0, n_channel) are ignored).
+ * first_chan, tau_ref: host; rsp_band: host, or device when on_device != 0. */
+int ppm_set_response(ppm_ctx* ctx, int n_channel, int band_w, const int32_t* first_chan,
+                     const double* rsp_band, int on_device, const double* tau_ref);
+
+/* S0-S5 of DESIGN.md: star/row scalars, cell mask, psi/lag lookup build, ring templates
+ * (Eq 38-44), shift-and-add with atmosphere interpolation (PAPER.md:417-430
+ * Eq 45-47).  params_dev [B][P]; flux_dev [B][n_phase][n_energy] photons cm^-2 s^-1 keV^-1
+ * (Eq 21); status_dev [B] (may be NULL). */
+int ppm_evaluate(ppm_ctx* ctx, const double* params_dev, int B, double* flux_dev, int32_t* status_dev);
+
+/* S6: C[b][k][c] = sum_e F_t[b][k][e] exp(-N_H20[b] tau_ref[e]) RSP0[e][c]  (Eq 22-23, 55).
+ * N_H20 is params[b][5].  counts_dev [B][n_phase][n_channel], counts/s. */
+int ppm_fold_response(ppm_ctx* ctx, const double* flux_dev, const double* params_dev, int B,
+                      double* counts_dev);
+
+/* S7: ln L_b = sum_{k,c} d ln m - m - lgamma(d+1),  m = exposure_s * C / n_phase + bkg[c]
+ * (reading R14).  0 ln 0 := 0; -inf if some m = 0 < d or C is NaN.
+ * data_dev [n_phase][n_channel]; bkg_dev [n_channel] or NULL; loglike_dev [B]. */
+int ppm_loglike(ppm_ctx* ctx, const double* counts_dev, int B, const double* data_dev,
+                const double* bkg_dev, double exposure_s, double* loglike_dev);
+
+/* Host-buffer variants: same computation, with the host->device copy of the inputs and the
+ * device->host copy of the result inside the call (they synchronise the stream).
+ * ppm_evaluate_host: params_host [B][P] -> flux_host [B][n_phase][n_energy], status_host [B] or NULL.
+ * ppm_loglike_host : params_host [B][P] -> evaluate + fold + ln L against data_dev / bkg_dev
+ *                    (device, set-up data) -> loglike_host [B], status_host [B] or NULL. */
+int ppm_evaluate_host(ppm_ctx* ctx, const double* params_host, int B, double* flux_host,
+                      int32_t* status_host);
+int ppm_loglike_host(ppm_ctx* ctx, const double* params_host, int B, const double* data_dev,
+                     const double* bkg_dev, double exposure_s, double* loglike_host,
+                     int32_t* status_host);
+
+/* Introspection of the intermediate device state left by the LAST ppm_evaluate call, for
+ * vector b of that call (tests compare each step with the oracle).  All outputs are host
+ * buffers; row index r = spot * n_theta + j.
+ *   rows    [n_rows][16]: theta, dcos, R_cm, u, f, coseta, sineta, beta, gamma, log10g,
+ *                         c_dt_cm (Eq 16), dOmega, alpha_max, psi_max, n_active, ring_visible
+ *   mask    [n_rows][n_phi] uint8, 1 = active cell (S1)
+ *   tmpl    [n_rows][4][n_fp+1]: F, z, phi_o, mu (S3, after the invisible-range fill)
+ *   lookup  evaluates the row's device-built lookup at n emission angles alpha[i]:
+ *           psi[i], dpsi_dalpha[i], lag[i] = (c Delta t - c delta t(R)) / R            (S2) */
+int ppm_debug_rows(ppm_ctx* ctx, int b, double* rows_host);
+int ppm_debug_mask(ppm_ctx* ctx, int b, uint8_t* mask_host);
+int ppm_debug_template(ppm_ctx* ctx, int b, double* tmpl_host);
+int ppm_debug_lookup(ppm_ctx* ctx, int b, int row, const double* alpha_host, int n,
+                     double* psi_host, double* dpsi_host, double* lag_host);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+int64_t ppm_launch_count(const ppm_ctx* ctx);
+/* Effective n_fp after defaulting. */
+int ppm_n_fp(const ppm_ctx* ctx);
+
+/* Register-resident DFMA chain on every SM: returns the measured FP64 FMA rate in flop/s
+ * (2 flop per DFMA) -- the roofline denominator of the cell kernel. */
+int ppm_measure_fp64_peak(int device, double* flops_per_s);
+
+const char* ppm_last_error(void); /* thread-local, static storage */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PPM_H_ */

@@ -1,0 +1,627 @@
+// ppm.cu -- C ABI (include/ppm.h) of the B200-native PPM hot path: context, table upload, launch
+// sequencing.  All arithmetic of the path runs in the kernels of ppm_geodesic.cuh / ppm_cells.cuh /
+// ppm_observe.cuh.  No CPU fallback.  Build: nvcc -gencode arch=compute_100a,code=sm_100a (see
+// paper_2510_07764_b200/_build.py).
+#include "ppm.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "ppm_common.cuh"
+#include "ppm_geodesic.cuh"
+#include "ppm_cells.cuh"
+#include "ppm_observe.cuh"
+
+using namespace ppm;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+void set_err(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            set_err("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);  \
+            return PPM_ERR_CUDA;                                                                   \
+        }                                                                                          \
+    } while (0)
+
+#define ARG(cond, msg)                     \
+    do {                                   \
+        if (!(cond)) {                     \
+            set_err("invalid argument: %s", msg); \
+            return PPM_ERR_ARG;            \
+        }                                  \
+    } while (0)
+
+// n-point Gauss-Legendre rule on [-1, 1]: Newton on P_n from the Chebyshev-like guess (textbook).
+void gauss_legendre(int n, double* x, double* w)
+{
+    for (int i = 0; i < n; ++i) {
+        long double z = cosl(3.14159265358979323846264338327950288L * (i + 0.75L) / (n + 0.5L)), pp = 1.0L;
+        for (int it = 0; it < 100; ++it) {
+            long double p1 = 1.0L, p2 = 0.0L;
+            for (int j = 1; j <= n; ++j) {
+                const long double p3 = p2;
+                p2 = p1;
+                p1 = ((2.0L * j - 1.0L) * z * p2 - (j - 1.0L) * p3) / j;
+            }
+            pp = n * (z * p1 - p2) / (z * z - 1.0L);
+            const long double dz = p1 / pp;
+            z -= dz;
+            if (fabsl(dz) < 1e-19L) {
+                p1 = 1.0L; p2 = 0.0L;
+                for (int j = 1; j <= n; ++j) {
+                    const long double p3 = p2;
+                    p2 = p1;
+                    p1 = ((2.0L * j - 1.0L) * z * p2 - (j - 1.0L) * p3) / j;
+                }
+                pp = n * (z * p1 - p2) / (z * z - 1.0L);
+                break;
+            }
+        }
+        x[i] = (double)z;
+        w[i] = (double)(2.0L / ((1.0L - z * z) * pp * pp));
+    }
+}
+
+template <typename T>
+int dev_alloc(T** p, size_t n)
+{
+    *p = nullptr;
+    if (n == 0) n = 1;
+    cudaError_t e = cudaMalloc((void**)p, n * sizeof(T));
+    if (e != cudaSuccess) {
+        set_err("cudaMalloc of %zu bytes failed: %s", n * sizeof(T), cudaGetErrorString(e));
+        return PPM_ERR_NOMEM;
+    }
+    return PPM_OK;
+}
+
+}  // namespace
+
+struct ppm_ctx {
+    ppm_config cfg;
+    cudaStream_t stream = nullptr;
+    int P = 0, RT = 0, n_fp = 0, SB = 1;          // params per vector, rows per vector, sub-batch size
+    int nchunk = 1, rows_per_chunk = 1, nw = 1, npg = 1, epl = 1, n_etile = 1;
+    int64_t launches = 0;
+    int last_nb = 0;
+    // energy grid
+    double *d_en = nullptr, *d_ue = nullptr, *d_le2 = nullptr;
+    std::vector<double> h_en;
+    // atmosphere
+    bool have_atm = false;
+    int nT = 0, ng = 0, nmu = 0, nx = 0;
+    double x0 = 0, hx = 1;
+    double *d_axT = nullptr, *d_axg = nullptr, *d_axmu = nullptr, *d_values = nullptr;
+    // response
+    bool have_rsp = false;
+    int n_channel = 0, band_w = 0;
+    int *d_first = nullptr, *d_elo = nullptr, *d_ehi = nullptr;
+    double *d_band = nullptr, *d_tau = nullptr;
+    // scratch (sub-batch sized)
+    StarD* d_stars = nullptr; SpotD* d_spots = nullptr; RowD* d_rows = nullptr; int* d_cells = nullptr;
+    double *d_lookup = nullptr, *d_tmpl = nullptr, *d_slices = nullptr, *d_partial = nullptr;
+    double* d_lgam = nullptr;
+    // host-variant staging
+    double *d_params_stage = nullptr, *d_flux_stage = nullptr, *d_ll_stage = nullptr, *d_counts_stage = nullptr;
+    int* d_status_stage = nullptr;
+    size_t cells_smem = 0;
+};
+
+extern "C" const char* ppm_last_error(void) { return g_err; }
+
+extern "C" int ppm_destroy(ppm_ctx* c)
+{
+    if (!c) return PPM_OK;
+    cudaSetDevice(c->cfg.device);
+    void* ptrs[] = {c->d_en, c->d_ue, c->d_le2, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
+                    c->d_ehi, c->d_band, c->d_tau, c->d_stars, c->d_spots, c->d_rows, c->d_cells, c->d_lookup,
+                    c->d_tmpl, c->d_slices, c->d_partial, c->d_lgam, c->d_params_stage, c->d_flux_stage,
+                    c->d_ll_stage, c->d_counts_stage, c->d_status_stage};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    delete c;
+    return PPM_OK;
+}
+
+static int alloc_scratch(ppm_ctx* c)
+{
+    const ppm_config& g = c->cfg;
+    const size_t rows = (size_t)c->SB * c->RT;
+    int rc;
+    if ((rc = dev_alloc(&c->d_stars, (size_t)c->SB))) return rc;
+    if ((rc = dev_alloc(&c->d_spots, (size_t)c->SB * g.n_spots))) return rc;
+    if ((rc = dev_alloc(&c->d_rows, rows))) return rc;
+    if ((rc = dev_alloc(&c->d_cells, rows * g.n_phi))) return rc;
+    if ((rc = dev_alloc(&c->d_lookup, rows * 2 * kNCheb))) return rc;
+    if ((rc = dev_alloc(&c->d_tmpl, rows * 4 * (c->n_fp + 1)))) return rc;
+    if ((rc = dev_alloc(&c->d_partial, (size_t)c->SB * c->nchunk * g.n_phase * g.n_energy))) return rc;
+    if ((rc = dev_alloc(&c->d_lgam, (size_t)1))) return rc;
+    return PPM_OK;
+}
+
+extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* stream, ppm_ctx** out)
+{
+    ARG(cfg && energies && out, "null pointer");
+    ARG(cfg->n_spots >= 1 && cfg->n_spots <= PPM_MAX_SPOTS, "n_spots must be 1..4");
+    ARG(cfg->n_theta >= 1 && cfg->n_phi >= 1 && cfg->n_phase >= 1 && cfg->n_energy >= 1, "grid sizes must be >= 1");
+    ARG(cfg->n_fp >= 0, "n_fp must be >= 0");
+    ARG(cfg->emission >= 0 && cfg->emission <= 2, "emission must be 0, 1 or 2");
+    ARG(cfg->precision == 0, "only precision = 0 (fp64) is implemented");
+    ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
+    for (int e = 0; e < cfg->n_energy; ++e) {
+        ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
+        if (e) ARG(energies[e] > energies[e - 1], "energies must be strictly increasing");
+    }
+    int ndev = 0;
+    CK(cudaGetDeviceCount(&ndev));
+    if (cfg->device < 0 || cfg->device >= ndev) { set_err("no CUDA device %d (found %d)", cfg->device, ndev); return PPM_ERR_CUDA; }
+    CK(cudaSetDevice(cfg->device));
+    ppm_ctx* c = new (std::nothrow) ppm_ctx;
+    if (!c) { set_err("out of host memory"); return PPM_ERR_NOMEM; }
+    c->cfg = *cfg;
+    c->stream = (cudaStream_t)stream;
+    c->P = 8 + 8 * cfg->n_spots;
+    c->RT = cfg->n_spots * cfg->n_theta;
+    c->n_fp = cfg->n_fp > 0 ? cfg->n_fp : std::max(192, 2 * cfg->n_phase);           // reading R2
+    c->h_en.assign(energies, energies + cfg->n_energy);
+    // launch geometry of the cell kernel
+    c->nw = std::min(16, cfg->n_phase);
+    c->npg = (cfg->n_phase + c->nw - 1) / c->nw;
+    const int need = (cfg->n_energy + 31) / 32;
+    const int epls[] = {1, 2, 4, 8, 10};
+    c->epl = 10;
+    for (int v : epls) if (v >= need) { c->epl = v; break; }
+    c->n_etile = (cfg->n_energy + 32 * c->epl - 1) / (32 * c->epl);
+    const double per_row = (double)cfg->n_phase * cfg->n_energy * 8.0;
+    c->rows_per_chunk = 1;
+    while ((double)((c->RT + c->rows_per_chunk - 1) / c->rows_per_chunk) * per_row > 96.0e6 && c->rows_per_chunk < c->RT)
+        c->rows_per_chunk *= 2;
+    c->nchunk = (c->RT + c->rows_per_chunk - 1) / c->rows_per_chunk;
+    // sub-batch: keep the per-launch scratch under ~1.5 GB
+    const double per_vec = (double)c->nchunk * per_row + (double)c->RT * (67.0 * 166.0 * 8.0 + 4.0 * (c->n_fp + 1) * 8.0 +
+                           cfg->n_phi * 4.0 + 2048.0);
+    c->SB = (int)std::max(1.0, std::min((double)cfg->max_batch, std::floor(1.5e9 / per_vec)));
+    c->SB = std::min(c->SB, 65535 / std::max(1, c->n_etile));
+    int rc = alloc_scratch(c);
+    if (rc) { ppm_destroy(c); return rc; }
+    // energy-derived constants: filled here for blackbody; refreshed by ppm_load_atmosphere (needs h)
+    if ((rc = dev_alloc(&c->d_en, (size_t)cfg->n_energy)) || (rc = dev_alloc(&c->d_ue, (size_t)cfg->n_energy)) ||
+        (rc = dev_alloc(&c->d_le2, (size_t)cfg->n_energy))) { ppm_destroy(c); return rc; }
+    std::vector<double> le2(cfg->n_energy);
+    for (int e = 0; e < cfg->n_energy; ++e) le2[e] = -std::log2(energies[e]);
+    CK(cudaMemcpyAsync(c->d_en, energies, sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_le2, le2.data(), sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream));
+    double glx[kNGL], glw[kNGL];
+    gauss_legendre(kNGL, glx, glw);
+    CK(cudaMemcpyToSymbolAsync(c_glx, glx, sizeof(glx), 0, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyToSymbolAsync(c_glw, glw, sizeof(glw), 0, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    *out = c;
+    return PPM_OK;
+}
+
+extern "C" int ppm_n_fp(const ppm_ctx* c) { return c ? c->n_fp : 0; }
+extern "C" int64_t ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const double* logg, int ng,
+                                   const double* mu, int nmu, const double* logx, int nx, const double* values,
+                                   int values_on_device)
+{
+    ARG(c && logT && logg && mu && logx && values, "null pointer");
+    ARG(nT >= 4 && ng >= 4 && nmu >= 4 && nx >= 4, "every table axis needs >= 4 nodes");
+    const double* axs[4] = {logT, logg, mu, logx};
+    const int ns[4] = {nT, ng, nmu, nx};
+    for (int a = 0; a < 4; ++a)
+        for (int i = 1; i < ns[a]; ++i) ARG(axs[a][i] > axs[a][i - 1], "table axes must be strictly increasing");
+    const double h = (logx[nx - 1] - logx[0]) / (nx - 1);
+    for (int i = 0; i < nx; ++i)
+        ARG(std::fabs(logx[i] - (logx[0] + h * i)) <= 1e-10 * std::fabs(h), "logx axis must be uniformly spaced");
+    CK(cudaSetDevice(c->cfg.device));
+    for (double** p : {&c->d_axT, &c->d_axg, &c->d_axmu, &c->d_values, &c->d_slices}) { if (*p) cudaFree(*p); *p = nullptr; }
+    c->have_atm = false;
+    int rc;
+    const size_t nval = (size_t)nT * ng * nmu * nx;
+    if ((rc = dev_alloc(&c->d_axT, (size_t)nT)) || (rc = dev_alloc(&c->d_axg, (size_t)ng)) ||
+        (rc = dev_alloc(&c->d_axmu, (size_t)nmu)) || (rc = dev_alloc(&c->d_values, nval)) ||
+        (rc = dev_alloc(&c->d_slices, (size_t)c->SB * c->RT * nmu * nx))) return rc;
+    CK(cudaMemcpyAsync(c->d_axT, logT, sizeof(double) * nT, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_axg, logg, sizeof(double) * ng, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_axmu, mu, sizeof(double) * nmu, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_values, values, sizeof(double) * nval,
+                       values_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    c->nT = nT; c->ng = ng; c->nmu = nmu; c->nx = nx; c->x0 = logx[0]; c->hx = h;
+    std::vector<double> ue(c->cfg.n_energy);
+    for (int e = 0; e < c->cfg.n_energy; ++e) ue[e] = std::log10(c->h_en[e]) / h;
+    CK(cudaMemcpyAsync(c->d_ue, ue.data(), sizeof(double) * ue.size(), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->have_atm = true;
+    return PPM_OK;
+}
+
+extern "C" int ppm_set_response(ppm_ctx* c, int n_channel, int band_w, const int32_t* first_chan,
+                                const double* rsp_band, int on_device, const double* tau_ref)
+{
+    ARG(c && first_chan && rsp_band && tau_ref, "null pointer");
+    ARG(n_channel >= 1 && band_w >= 1, "n_channel and band_w must be >= 1");
+    const int nE = c->cfg.n_energy;
+    CK(cudaSetDevice(c->cfg.device));
+    for (void** p : {(void**)&c->d_first, (void**)&c->d_elo, (void**)&c->d_ehi, (void**)&c->d_band, (void**)&c->d_tau,
+                     (void**)&c->d_counts_stage}) { if (*p) cudaFree(*p); *p = nullptr; }
+    c->have_rsp = false;
+    // per channel: smallest range [e_lo, e_hi) containing every energy whose band covers it
+    std::vector<int> elo(n_channel, nE), ehi(n_channel, 0);
+    for (int e = 0; e < nE; ++e)
+        for (int w = 0; w < band_w; ++w) {
+            const long ch = (long)first_chan[e] + w;
+            if (ch < 0 || ch >= n_channel) continue;
+            elo[ch] = std::min(elo[ch], e);
+            ehi[ch] = std::max(ehi[ch], e + 1);
+        }
+    for (int ch = 0; ch < n_channel; ++ch) if (elo[ch] > ehi[ch]) elo[ch] = ehi[ch] = 0;
+    int rc;
+    if ((rc = dev_alloc(&c->d_first, (size_t)nE)) || (rc = dev_alloc(&c->d_elo, (size_t)n_channel)) ||
+        (rc = dev_alloc(&c->d_ehi, (size_t)n_channel)) || (rc = dev_alloc(&c->d_band, (size_t)nE * band_w)) ||
+        (rc = dev_alloc(&c->d_tau, (size_t)nE))) return rc;
+    CK(cudaMemcpyAsync(c->d_first, first_chan, sizeof(int) * nE, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_elo, elo.data(), sizeof(int) * n_channel, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_ehi, ehi.data(), sizeof(int) * n_channel, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_band, rsp_band, sizeof(double) * nE * band_w,
+                       on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_tau, tau_ref, sizeof(double) * nE, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->n_channel = n_channel; c->band_w = band_w;
+    c->have_rsp = true;
+    return PPM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// evaluation
+// ------------------------------------------------------------------------------------------------
+template <int EPL, int MODE>
+static int launch_cells(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    static thread_local size_t configured = 0;
+    if (smem > configured) {
+        CK(cudaFuncSetAttribute(k_cells<EPL, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    k_cells<EPL, MODE><<<grid, threads, smem, c->stream>>>(a);
+    return PPM_OK;
+}
+
+template <int MODE>
+static int dispatch_cells(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    switch (c->epl) {
+    case 1:  return launch_cells<1, MODE>(c, a, grid, threads, smem);
+    case 2:  return launch_cells<2, MODE>(c, a, grid, threads, smem);
+    case 4:  return launch_cells<4, MODE>(c, a, grid, threads, smem);
+    case 8:  return launch_cells<8, MODE>(c, a, grid, threads, smem);
+    default: return launch_cells<10, MODE>(c, a, grid, threads, smem);
+    }
+}
+
+static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* flux_dev, int32_t* status_dev)
+{
+    const ppm_config& g = c->cfg;
+    const bool table = g.emission != PPM_EMISSION_BLACKBODY;
+    GeoArgs G;
+    G.params = params_dev; G.nb = nb; G.P = c->P; G.n_spots = g.n_spots; G.n_theta = g.n_theta; G.n_phi = g.n_phi;
+    G.n_phase = g.n_phase; G.n_fp = c->n_fp; G.oblate = g.oblate; G.emission = g.emission;
+    G.stars = c->d_stars; G.spots = c->d_spots; G.rows = c->d_rows; G.cells = c->d_cells;
+    G.lookup = c->d_lookup; G.tmpl = c->d_tmpl;
+    G.axT = c->d_axT; G.nT = c->nT; G.axg = c->d_axg; G.ng = c->ng;
+    const int rows = nb * c->RT;
+    k_star<<<(nb + 63) / 64, 64, 0, c->stream>>>(G);
+    k_rows<<<rows, 128, 0, c->stream>>>(G);
+    k_lookup<<<rows, kNCheb, 0, c->stream>>>(G);
+    const size_t tsm = sizeof(double) * (2 * kNCheb + 4 * (size_t)(c->n_fp + 1));
+    if (tsm > 48 * 1024) CK(cudaFuncSetAttribute(k_template, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
+    k_template<<<rows, 128, tsm, c->stream>>>(G);
+    c->launches += 4;
+    if (table) {
+        SliceArgs S;
+        S.spots = c->d_spots; S.rows = c->d_rows; S.values = c->d_values; S.slices = c->d_slices;
+        S.n_theta = g.n_theta; S.nT = c->nT; S.ng = c->ng; S.nmu = c->nmu; S.nx = c->nx;
+        dim3 sg((c->nmu * c->nx + 255) / 256, rows);
+        k_slice<<<sg, 256, 0, c->stream>>>(S);
+        c->launches += 1;
+    }
+    CellArgs A;
+    A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
+    A.slices = c->d_slices; A.axmu = c->d_axmu; A.ue = c->d_ue; A.le2 = c->d_le2; A.en = c->d_en;
+    A.partial = c->d_partial;
+    A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
+    A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;
+    A.n_fp = c->n_fp; A.nE = g.n_energy;
+    A.nmu = table ? c->nmu : 0; A.nx = table ? c->nx : 0;
+    A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
+    A.x_linedge = g.emission == PPM_EMISSION_TABLE_MIXED ? 1 : 0;
+    A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
+    const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu + (size_t)c->nw * A.nx);
+    if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
+    dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
+    int rc = table ? dispatch_cells<1>(c, A, grid, c->nw * 32, smem) : dispatch_cells<0>(c, A, grid, c->nw * 32, smem);
+    if (rc) return rc;
+    const int n_out = g.n_phase * g.n_energy;
+    dim3 rg((n_out + 255) / 256, nb);
+    k_reduce<<<rg, 256, 0, c->stream>>>(c->d_partial, c->d_stars, c->nchunk, n_out, flux_dev, status_dev);
+    c->launches += 2;
+    CK(cudaGetLastError());
+    c->last_nb = nb;
+    return PPM_OK;
+}
+
+extern "C" int ppm_evaluate(ppm_ctx* c, const double* params_dev, int B, double* flux_dev, int32_t* status_dev)
+{
+    ARG(c && params_dev && flux_dev, "null pointer");
+    ARG(B >= 0, "B must be >= 0");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
+        set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE;
+    }
+    CK(cudaSetDevice(c->cfg.device));
+    const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy;
+    for (int b0 = 0; b0 < B; b0 += c->SB) {
+        const int nb = std::min(c->SB, B - b0);
+        int rc = evaluate_sub(c, params_dev + (size_t)b0 * c->P, nb, flux_dev + (size_t)b0 * fstride,
+                              status_dev ? status_dev + b0 : nullptr);
+        if (rc) return rc;
+    }
+    return PPM_OK;
+}
+
+extern "C" int ppm_fold_response(ppm_ctx* c, const double* flux_dev, const double* params_dev, int B, double* counts_dev)
+{
+    ARG(c && flux_dev && params_dev && counts_dev, "null pointer");
+    ARG(B >= 0, "B must be >= 0");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
+    if (B == 0) return PPM_OK;
+    CK(cudaSetDevice(c->cfg.device));
+    FoldArgs F;
+    F.flux = flux_dev; F.params = params_dev; F.band = c->d_band; F.tau = c->d_tau; F.first = c->d_first;
+    F.e_lo = c->d_elo; F.e_hi = c->d_ehi; F.counts = counts_dev;
+    F.P = c->P; F.n_phase = c->cfg.n_phase; F.nE = c->cfg.n_energy; F.n_channel = c->n_channel; F.band_w = c->band_w;
+    const size_t smem = sizeof(double) * c->cfg.n_energy;
+    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(k_fold, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    for (int b0 = 0; b0 < B; b0 += 65535) {
+        const int nb = std::min(65535, B - b0);
+        FoldArgs Fs = F;
+        Fs.flux = flux_dev + (size_t)b0 * F.n_phase * F.nE;
+        Fs.params = params_dev + (size_t)b0 * F.P;
+        Fs.counts = counts_dev + (size_t)b0 * F.n_phase * F.n_channel;
+        dim3 grid((c->n_channel + 127) / 128, c->cfg.n_phase, nb);
+        k_fold<<<grid, 128, smem, c->stream>>>(Fs);
+        c->launches += 1;
+    }
+    CK(cudaGetLastError());
+    return PPM_OK;
+}
+
+extern "C" int ppm_loglike(ppm_ctx* c, const double* counts_dev, int B, const double* data_dev, const double* bkg_dev,
+                           double exposure_s, double* loglike_dev)
+{
+    ARG(c && counts_dev && data_dev && loglike_dev, "null pointer");
+    ARG(B >= 0, "B must be >= 0");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
+    if (B == 0) return PPM_OK;
+    CK(cudaSetDevice(c->cfg.device));
+    k_loglike<<<1, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
+                                        nullptr, 1, c->d_lgam);
+    k_loglike<<<B, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
+                                        c->d_lgam, 0, loglike_dev);
+    c->launches += 2;
+    CK(cudaGetLastError());
+    return PPM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-buffer variants (copies inside the call)
+// ------------------------------------------------------------------------------------------------
+static int ensure_stage(ppm_ctx* c)
+{
+    int rc;
+    const size_t mb = (size_t)c->cfg.max_batch;
+    if (!c->d_params_stage && (rc = dev_alloc(&c->d_params_stage, mb * c->P))) return rc;
+    if (!c->d_status_stage && (rc = dev_alloc(&c->d_status_stage, mb))) return rc;
+    if (!c->d_ll_stage && (rc = dev_alloc(&c->d_ll_stage, mb))) return rc;
+    return PPM_OK;
+}
+
+extern "C" int ppm_evaluate_host(ppm_ctx* c, const double* params_host, int B, double* flux_host, int32_t* status_host)
+{
+    ARG(c && params_host && flux_host, "null pointer");
+    ARG(B >= 0, "B must be >= 0");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    CK(cudaSetDevice(c->cfg.device));
+    int rc = ensure_stage(c);
+    if (rc) return rc;
+    const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy;
+    if (!c->d_flux_stage && (rc = dev_alloc(&c->d_flux_stage, (size_t)c->SB * fstride))) return rc;
+    CK(cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * c->P, cudaMemcpyHostToDevice, c->stream));
+    if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
+        set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE;
+    }
+    for (int b0 = 0; b0 < B; b0 += c->SB) {
+        const int nb = std::min(c->SB, B - b0);
+        rc = evaluate_sub(c, c->d_params_stage + (size_t)b0 * c->P, nb, c->d_flux_stage, c->d_status_stage + b0);
+        if (rc) return rc;
+        CK(cudaMemcpyAsync(flux_host + (size_t)b0 * fstride, c->d_flux_stage, sizeof(double) * nb * fstride,
+                           cudaMemcpyDeviceToHost, c->stream));
+    }
+    if (status_host)
+        CK(cudaMemcpyAsync(status_host, c->d_status_stage, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return PPM_OK;
+}
+
+extern "C" int ppm_loglike_host(ppm_ctx* c, const double* params_host, int B, const double* data_dev,
+                                const double* bkg_dev, double exposure_s, double* loglike_host, int32_t* status_host)
+{
+    ARG(c && params_host && data_dev && loglike_host, "null pointer");
+    ARG(B >= 0, "B must be >= 0");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
+    if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
+        set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE;
+    }
+    CK(cudaSetDevice(c->cfg.device));
+    int rc = ensure_stage(c);
+    if (rc) return rc;
+    const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy;
+    const size_t cstride = (size_t)c->cfg.n_phase * c->n_channel;
+    if (!c->d_flux_stage && (rc = dev_alloc(&c->d_flux_stage, (size_t)c->SB * fstride))) return rc;
+    if (!c->d_counts_stage && (rc = dev_alloc(&c->d_counts_stage, (size_t)c->SB * cstride))) return rc;
+    CK(cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * c->P, cudaMemcpyHostToDevice, c->stream));
+    for (int b0 = 0; b0 < B; b0 += c->SB) {
+        const int nb = std::min(c->SB, B - b0);
+        const double* pd = c->d_params_stage + (size_t)b0 * c->P;
+        if ((rc = evaluate_sub(c, pd, nb, c->d_flux_stage, c->d_status_stage + b0))) return rc;
+        if ((rc = ppm_fold_response(c, c->d_flux_stage, pd, nb, c->d_counts_stage))) return rc;
+        if ((rc = ppm_loglike(c, c->d_counts_stage, nb, data_dev, bkg_dev, exposure_s, c->d_ll_stage + b0))) return rc;
+    }
+    CK(cudaMemcpyAsync(loglike_host, c->d_ll_stage, sizeof(double) * B, cudaMemcpyDeviceToHost, c->stream));
+    if (status_host)
+        CK(cudaMemcpyAsync(status_host, c->d_status_stage, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return PPM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// introspection (tests) and the FP64 peak probe
+// ------------------------------------------------------------------------------------------------
+static int debug_check(ppm_ctx* c, int b)
+{
+    ARG(c, "null context");
+    if (b < 0 || b >= c->last_nb) {
+        set_err("vector %d is not in the last evaluated sub-batch (size %d)", b, c->last_nb);
+        return PPM_ERR_ARG;
+    }
+    CK(cudaSetDevice(c->cfg.device));
+    CK(cudaStreamSynchronize(c->stream));
+    return PPM_OK;
+}
+
+extern "C" int ppm_debug_rows(ppm_ctx* c, int b, double* out)
+{
+    int rc = debug_check(c, b);
+    if (rc) return rc;
+    ARG(out, "null pointer");
+    std::vector<RowD> h(c->RT);
+    CK(cudaMemcpy(h.data(), c->d_rows + (size_t)b * c->RT, sizeof(RowD) * c->RT, cudaMemcpyDeviceToHost));
+    for (int r = 0; r < c->RT; ++r) {
+        const RowD& q = h[r];
+        const double v[16] = {q.theta, q.dcos, q.R, q.u, q.f, q.coseta, q.sineta, q.beta, q.gamma, q.log10g, q.c_dt,
+                              q.dOmega, q.alpha_max, q.psi_max, (double)q.n_active, (double)q.visible};
+        std::memcpy(out + (size_t)r * 16, v, sizeof(v));
+    }
+    return PPM_OK;
+}
+
+extern "C" int ppm_debug_mask(ppm_ctx* c, int b, uint8_t* out)
+{
+    int rc = debug_check(c, b);
+    if (rc) return rc;
+    ARG(out, "null pointer");
+    const int nphi = c->cfg.n_phi;
+    std::vector<RowD> h(c->RT);
+    std::vector<int> cl((size_t)c->RT * nphi);
+    CK(cudaMemcpy(h.data(), c->d_rows + (size_t)b * c->RT, sizeof(RowD) * c->RT, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(cl.data(), c->d_cells + (size_t)b * c->RT * nphi, sizeof(int) * cl.size(), cudaMemcpyDeviceToHost));
+    std::memset(out, 0, (size_t)c->RT * nphi);
+    for (int r = 0; r < c->RT; ++r)
+        for (int i = 0; i < h[r].n_active; ++i) out[(size_t)r * nphi + cl[(size_t)r * nphi + i]] = 1;
+    return PPM_OK;
+}
+
+extern "C" int ppm_debug_template(ppm_ctx* c, int b, double* out)
+{
+    int rc = debug_check(c, b);
+    if (rc) return rc;
+    ARG(out, "null pointer");
+    const size_t n1 = (size_t)c->n_fp + 1, per = 4 * n1;
+    std::vector<RowD> h(c->RT);
+    CK(cudaMemcpy(h.data(), c->d_rows + (size_t)b * c->RT, sizeof(RowD) * c->RT, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(out, c->d_tmpl + (size_t)b * c->RT * per, sizeof(double) * c->RT * per, cudaMemcpyDeviceToHost));
+    for (int r = 0; r < c->RT; ++r)                      // rows that were skipped hold stale scratch: report zeros
+        if (h[r].n_active == 0) std::memset(out + (size_t)r * per, 0, sizeof(double) * per);
+    return PPM_OK;
+}
+
+extern "C" int ppm_debug_lookup(ppm_ctx* c, int b, int row, const double* alpha, int n, double* psi, double* dpsi,
+                                double* lag)
+{
+    int rc = debug_check(c, b);
+    if (rc) return rc;
+    ARG(alpha && psi && dpsi && lag && n >= 1, "null pointer or n < 1");
+    ARG(row >= 0 && row < c->RT, "row out of range");
+    RowD h;
+    CK(cudaMemcpy(&h, c->d_rows + (size_t)b * c->RT + row, sizeof(RowD), cudaMemcpyDeviceToHost));
+    if (h.n_active == 0) { set_err("row %d has no active cell: no lookup was built", row); return PPM_ERR_STATE; }
+    double* d = nullptr;
+    if ((rc = dev_alloc(&d, (size_t)4 * n))) return rc;
+    cudaError_t e = cudaMemcpy(d, alpha, sizeof(double) * n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_lookup_eval<<<(n + 127) / 128, 128, 0, c->stream>>>(c->d_lookup + ((size_t)b * c->RT + row) * 2 * kNCheb,
+                                                              h.alpha_max, d, n, d + n, d + 2 * n, d + 3 * n);
+        c->launches += 1;
+        e = cudaStreamSynchronize(c->stream);
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(psi, d + n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(dpsi, d + 2 * n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(lag, d + 3 * n, sizeof(double) * n, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) { set_err("ppm_debug_lookup: %s", cudaGetErrorString(e)); return PPM_ERR_CUDA; }
+    return PPM_OK;
+}
+
+extern "C" int ppm_measure_fp64_peak(int device, double* flops_per_s)
+{
+    ARG(flops_per_s, "null pointer");
+    CK(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, device));
+    double* d = nullptr;
+    int rc = dev_alloc(&d, (size_t)1);
+    if (rc) return rc;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 4096;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        CK(cudaEventRecord(e0, 0));
+        k_dfma_peak<<<blocks, threads>>>(d, iters, 1.0 + rep);
+        CK(cudaEventRecord(e1, 0));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        const double fl = (double)blocks * threads * 8.0 * 8.0 * iters * 2.0 / (ms * 1.0e-3);
+        if (rep > 0 && fl > best) best = fl;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    *flops_per_s = best;
+    return PPM_OK;
+}
