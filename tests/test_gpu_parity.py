@@ -1,0 +1,132 @@
+"""-m gpu: the CUDA path (through the C ABI) against the oracle, element by element on the same
+seeded inputs.  Bar (BASELINE.json north_star): max relative error per (phase, energy) bin 1e-9."""
+import numpy as np
+import pytest
+
+import gen
+import oracle as o
+from gpu_common import gpu_flux, make_ctx, max_rel_err, oracle_flux
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-9
+
+
+def test_c1_tiny_full():
+    conf = gen.config_c1()
+    g, st, _ = gpu_flux(conf)
+    ref, so = oracle_flux(conf)
+    assert st[0] == 0 and so == 0
+    assert ref.max() > 0
+    assert max_rel_err(g[0], ref) <= TOL
+
+
+def test_c2_cubic_full():
+    conf = gen.config_c2()
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+def test_c3_mixed_reduced_and_ragged():
+    conf = gen.config_c3(n_cells=40, n_phase=37, n_energy=77)     # ragged tails in every dimension
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+def test_c3_full_size_sampled_phases():
+    conf = gen.config_c3()
+    g, st, _ = gpu_flux(conf)
+    sel = [0, 67, 128, 201]
+    ref, _ = oracle_flux(conf, phase_sel=sel)
+    assert st[0] == 0 and max_rel_err(g[0][sel], ref) <= TOL
+
+
+def test_c4_extreme_reduced():
+    conf = gen.config_c4(n_cells=48, n_phase=64, n_energy=96)
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+def test_target_full_size_sampled_phases():
+    conf = gen.config_t()
+    g, st, _ = gpu_flux(conf)
+    sel = [3, 77]
+    ref, _ = oracle_flux(conf, phase_sel=sel)
+    assert st[0] == 0 and max_rel_err(g[0][sel], ref) <= TOL
+    # properties that hold at any size: non-negative, finite, periodic continuity of the profile
+    assert np.all(np.isfinite(g[0])) and np.all(g[0] >= 0)
+
+
+def test_batch_matches_single_and_status_codes():
+    conf = gen.config_c5(n_vec=5, n_cells=24, n_phase=16, n_energy=40)
+    P = conf["params"].copy()
+    P[1, 1] = 4.0            # R_eq = 4 km: compactness out of domain -> status 1
+    P[3, 10] = -0.5          # zeta < 0 -> status 4
+    conf["params"] = P
+    g, st, ctx = gpu_flux(conf)
+    assert list(st) == [0, 1, 0, 4, 0]
+    assert np.all(np.isnan(g[1])) and np.all(np.isnan(g[3]))
+    for b in (0, 2, 4):
+        ref, so = oracle_flux(conf, b)
+        assert so == 0 and max_rel_err(g[b], ref) <= TOL
+    assert o.evaluate(conf["cfg"], conf["energies"], P[1], None if conf["cfg"]["emission"] == 0 else
+                      __import__("gpu_common").oracle_atm())[1] == 1
+    # host-buffer entry point gives the same numbers
+    gh, sh = ctx.evaluate_host(P)
+    assert np.array_equal(sh, st) and np.array_equal(np.isnan(gh), np.isnan(g))
+    assert np.array_equal(gh[[0, 2, 4]], g[[0, 2, 4]])             # deterministic: bit-identical re-run
+
+
+def test_occluded_spot_is_exactly_zero_and_empty_batch():
+    import torch
+    E = gen.logspace(0.3, 3.0, 8)
+    cfg = dict(n_spots=1, n_theta=8, n_phi=8, n_phase=16, n_fp=192, emission=0, oblate=0)
+    p = gen.pack_params(1.4, 12.0, 200.0, np.cos(0.3), 0.2, spots=[(2.9, 0.0, 0.1, 6.5)])     # pin P8 geometry
+    conf = dict(cfg=cfg, energies=E, params=p[None, :])
+    g, st, ctx = gpu_flux(conf)
+    assert st[0] == 0 and np.all(g == 0.0)
+    ref, _ = oracle_flux(conf)
+    assert np.all(ref == 0.0)
+    empty = torch.empty((0, ctx.P), dtype=torch.float64, device="cuda")
+    f, s = ctx.evaluate(empty)
+    assert f.shape[0] == 0
+    import paper_2510_07764_b200 as ppm
+    with pytest.raises(ppm.PPMError):
+        ctx.evaluate(torch.zeros((2, ctx.P), dtype=torch.float64, device="cuda"))   # B > max_batch
+    with pytest.raises(ppm.PPMError):
+        ppm.PPM(dict(cfg, emission=2), E).evaluate(torch.zeros((1, ctx.P), dtype=torch.float64, device="cuda"))
+
+
+def test_fold_and_loglike():
+    import torch
+    conf = gen.config_c5(n_vec=3, n_cells=16, n_phase=8, n_energy=300)
+    rsp = gen.synthetic_response(conf["energies"])
+    ctx = make_ctx(conf)
+    ctx.set_response(rsp["n_channel"], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"])
+    p = torch.as_tensor(conf["params"], device="cuda")
+    flux, _ = ctx.evaluate(p)
+    counts = ctx.fold_response(flux, p)
+    fh = flux.cpu().numpy()
+    ch = counts.cpu().numpy()
+    cref = [o.fold(fh[b], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"], conf["params"][b, 5], rsp["n_channel"])
+            for b in range(3)]
+    for b in range(3):
+        assert max_rel_err(ch[b], cref[b]) <= 1e-13
+    expo = 1e6 / (cref[0].sum() / 8)
+    bkg = np.full(rsp["n_channel"], 0.05 * 1e6 / (8 * rsp["n_channel"]))
+    rng = np.random.default_rng(11)
+    data = rng.poisson(expo * cref[0] / 8 + bkg).astype(np.float64)
+    ll = ctx.loglike(counts, torch.as_tensor(data, device="cuda"), torch.as_tensor(bkg, device="cuda"), expo)
+    ll = ll.cpu().numpy()
+    for b in range(3):
+        ref = o.loglike(cref[b], data, bkg, expo)
+        assert abs(ll[b] - ref) <= 1e-9 * data.sum(), (b, ll[b], ref)
+    # host-buffer one-call path
+    llh, sth = ctx.loglike_host(conf["params"], torch.as_tensor(data, device="cuda"),
+                                torch.as_tensor(bkg, device="cuda"), expo)
+    assert np.array_equal(llh, ll) and np.all(sth == 0)
+    # -inf when the model is zero where data are not
+    ll0 = ctx.loglike(torch.zeros_like(counts), torch.as_tensor(data, device="cuda"), None, expo).cpu().numpy()
+    assert np.all(np.isneginf(ll0))
