@@ -372,8 +372,10 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
 
 extern "C" int ppm_evaluate(ppm_ctx* c, const double* params_dev, int B, double* flux_dev, int32_t* status_dev)
 {
-    ARG(c && params_dev && flux_dev, "null pointer");
+    ARG(c, "null context");
     ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;                                   // empty batch: nothing to do, pointers may be NULL
+    ARG(params_dev && flux_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
     if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
         set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE;
@@ -391,8 +393,10 @@ extern "C" int ppm_evaluate(ppm_ctx* c, const double* params_dev, int B, double*
 
 extern "C" int ppm_fold_response(ppm_ctx* c, const double* flux_dev, const double* params_dev, int B, double* counts_dev)
 {
-    ARG(c && flux_dev && params_dev && counts_dev, "null pointer");
+    ARG(c, "null context");
     ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;
+    ARG(flux_dev && params_dev && counts_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
     if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
     if (B == 0) return PPM_OK;
@@ -420,8 +424,10 @@ extern "C" int ppm_fold_response(ppm_ctx* c, const double* flux_dev, const doubl
 extern "C" int ppm_loglike(ppm_ctx* c, const double* counts_dev, int B, const double* data_dev, const double* bkg_dev,
                            double exposure_s, double* loglike_dev)
 {
-    ARG(c && counts_dev && data_dev && loglike_dev, "null pointer");
+    ARG(c, "null context");
     ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;
+    ARG(counts_dev && data_dev && loglike_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
     if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
     if (B == 0) return PPM_OK;
@@ -450,8 +456,10 @@ static int ensure_stage(ppm_ctx* c)
 
 extern "C" int ppm_evaluate_host(ppm_ctx* c, const double* params_host, int B, double* flux_host, int32_t* status_host)
 {
-    ARG(c && params_host && flux_host, "null pointer");
+    ARG(c, "null context");
     ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;
+    ARG(params_host && flux_host, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
     CK(cudaSetDevice(c->cfg.device));
     int rc = ensure_stage(c);
@@ -478,8 +486,10 @@ extern "C" int ppm_evaluate_host(ppm_ctx* c, const double* params_host, int B, d
 extern "C" int ppm_loglike_host(ppm_ctx* c, const double* params_host, int B, const double* data_dev,
                                 const double* bkg_dev, double exposure_s, double* loglike_host, int32_t* status_host)
 {
-    ARG(c && params_host && data_dev && loglike_host, "null pointer");
+    ARG(c, "null context");
     ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;
+    ARG(params_host && data_dev && loglike_host, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
     if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
     if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
