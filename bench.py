@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the PPM hot path (pulse-profile evaluations per second).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ppm|reference]
+                    [--workload C5|T|C2|C3|C4] [--batch B] [--no-cpu-baseline]
+
+A *step* is one pass of the whole hot path S0..S7 over one batch of B seeded
+parameter vectors: ppm_evaluate -> ppm_fold_response -> ppm_loglike, everything through the C ABI of
+include/ppm.h.  Default workload: B = 8 vectors of BASELINE.json configs[4] (C5; each vector is the
+north-star target evaluation T: 2 spots x 256x256 cells, 128 phases x 300 energies, mixed-order
+interpolation on the synthetic 35x11x67x166 table, fold to 1500 channels, Poisson ln L).
+With N > 1 (torchrun, one rank per GPU) every rank takes its own B vectors of C5 -- independent
+units, no data-path collective ("scaling": "weak"); the time is the max over ranks.
+
+One JSON line is printed by rank 0.  `value` has the parameter batch resident in HBM; `e2e` runs
+ppm_loglike_host (host parameter buffer in, host ln L out, copies inside the timed region).
+`roofline` is for the dominant kernel k_cells: bound "alu" (FP64 pipe), algorithmic flops = 86 per
+accumulated (cell, phase, energy) triple / the kernel's own
+CUDA-event time measured inside the library on its launch stream.  `cpu_baseline` times the CPU
+oracle as it stands on a bounded sample of the same workload (rank 0, N = 1 only).
+
+--impl reference: there is no reference implementation (the paper's code is not available); per
+the task contract the reference arm is the CPU oracle, timed on the host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gen  # noqa: E402
+
+FLOP_PER_TRIPLE = 86.0          # SURVEY.md 8(d) accounting constant (FMA = 2 flop)
+# nominal FP64 vector peak: 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
+FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
+METRIC = "pulse-profile evaluations per second"
+UNIT = "evals/s"
+
+
+def workload(name, batch, rank):
+    """-> (conf dict with `batch` parameter vectors for this rank, description)."""
+    if name in ("C5", "T"):
+        B = 1 if name == "T" else batch
+        conf = gen.config_c5(n_vec=B * (rank + 1))
+        conf["params"] = np.ascontiguousarray(conf["params"][B * rank:B * (rank + 1)])
+        desc = ("BASELINE.json configs[4] (C5 batched likelihood): %d seeded prior vectors per GPU, each 2 spots x "
+                "256x256 cells, 128 phases x 300 energies 0.2-12 keV, mixed-order interpolation on the synthetic "
+                "35x11x67x166 table, banded fold 300 -> 1500 channels, Poisson ln L" % B)
+        if name == "T":
+            desc = "north-star target T = vector 0 of C5 evaluated alone; " + desc
+        return conf, desc
+    conf = {"C2": gen.config_c2, "C3": gen.config_c3, "C4": gen.config_c4}[name]()
+    conf["params"] = np.ascontiguousarray(np.repeat(conf["params"], batch, axis=0))
+    return conf, "BASELINE.json config %s, batch of %d identical vectors" % (name, batch)
+
+
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason samples during the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); smax.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=max(pw))
+        return out
+
+
+def oracle_sample(conf, n_extra=4):
+    """Time the CPU oracle, as it stands, on vector 0 of the workload: one run on 1 output phase and
+    one on 1 + n_extra phases (the per-row template work is paid once per run, the shift-and-add
+    scales with the phases), fold + ln L on the sampled phases; the full-evaluation time is the
+    linear extrapolation to n_phase phases.  -> dict(value evals/s, seconds, cores, sample)."""
+    import oracle as o
+    cfg, E, p = conf["cfg"], conf["energies"], conf["params"][0]
+    atm = o.Atmosphere(*gen.synthetic_atmosphere()) if cfg["emission"] else None
+    nph = cfg["n_phase"]
+    sel1 = [nph // 3]
+    sel2 = sel1 + [(nph // 3 + (i + 1) * nph // (n_extra + 1)) % nph for i in range(n_extra)]
+    rsp = gen.synthetic_response(E) if len(E) == 300 else None
+    t0 = time.perf_counter()
+    o.evaluate(cfg, E, p, atm, phase_sel=sel1)
+    t1 = time.perf_counter()
+    f2, _ = o.evaluate(cfg, E, p, atm, phase_sel=sel2)
+    if rsp is not None:
+        c = o.fold(f2, rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"], p[5], rsp["n_channel"])
+        o.loglike(c, np.ones_like(c), None, 1.0)
+    t2 = time.perf_counter()
+    d1, d2 = t1 - t0, t2 - t1
+    per_phase = max(d2 - d1, 0.0) / n_extra
+    full = d1 + per_phase * (nph - 1)
+    return dict(value=1.0 / full, seconds=d1 + d2, cores=o.num_threads(), full_eval_s=full,
+                sample="vector 0: oracle run on 1 and on %d of %d output phases (%.1f s + %.1f s), full evaluation "
+                       "extrapolated linearly in phases to %.1f s" % (1 + n_extra, nph, d1, d2, full))
+
+
+def run_reference(args, rank):
+    """Reference arm = the CPU oracle (rank 0 only)."""
+    if rank != 0:
+        return
+    conf, desc = workload(args.workload, args.batch, 0)
+    for _ in range(args.warmup):
+        oracle_sample(conf, n_extra=1)
+    vals, secs, last = [], 0.0, None
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        last = oracle_sample(conf, n_extra=2)
+        vals.append(last["value"])
+        secs += last["seconds"]
+    wall = time.perf_counter() - t0
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(args.steps, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "note": "reference arm = CPU oracle (oracle/ppm_oracle.c, direct quadrature), "
+                                                  "each step a bounded sample: " + last["sample"]},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+                             "sample": last["sample"]},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ppm", choices=["ppm", "reference"])
+    ap.add_argument("--workload", default="C5", choices=["C5", "T", "C2", "C3", "C4"])
+    ap.add_argument("--batch", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import paper_2510_07764_b200 as ppm
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the PPM hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    conf, desc = workload(args.workload, args.batch, rank)
+    cfg, E = conf["cfg"], conf["energies"]
+    B = conf["params"].shape[0]
+    ctx = ppm.PPM(cfg, E, max_batch=B, device=local)
+    if cfg["emission"]:
+        ctx.load_atmosphere(*gen.synthetic_atmosphere())
+    rsp = gen.synthetic_response(E)
+    ctx.set_response(rsp["n_channel"], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"])
+    data_h, bkg_h = gen.synthetic_counts(cfg["n_phase"], rsp["n_channel"])
+    data = torch.as_tensor(data_h, device=dev)
+    bkg = torch.as_tensor(bkg_h, device=dev)
+    exposure = 1.0e6
+    params = torch.as_tensor(conf["params"], dtype=torch.float64, device=dev).contiguous()
+    params_pinned = torch.as_tensor(conf["params"], dtype=torch.float64).contiguous().pin_memory()
+    flux = torch.empty((B, cfg["n_phase"], len(E)), dtype=torch.float64, device=dev)
+    status = torch.empty((B,), dtype=torch.int32, device=dev)
+    counts = torch.empty((B, cfg["n_phase"], rsp["n_channel"]), dtype=torch.float64, device=dev)
+    ll = torch.empty((B,), dtype=torch.float64, device=dev)
+    ll_host = np.empty((B,))
+    st_host = np.empty((B,), dtype=np.int32)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def step():
+        ctx.evaluate(params, flux, status)
+        ctx.fold_response(flux, params, counts)
+        ctx.loglike(counts, data, bkg, exposure, ll)
+
+    def step_e2e():
+        ctx.loglike_host(params_pinned.numpy(), data, bkg, exposure, ll_host, st_host)
+
+    def sync():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, k):
+        """K steps between two events on the launch stream; L2 flushed before every step."""
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * k)]
+        sync()
+        t0 = time.perf_counter()
+        for i in range(k):
+            flush.zero_()
+            ev[2 * i].record()
+            fn()
+            ev[2 * i + 1].record()
+        sync()
+        wall = time.perf_counter() - t0
+        per = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(k)]
+        total = ev[0].elapsed_time(ev[2 * k - 1])
+        t = torch.tensor([total, wall * 1e3], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t[0]), float(t[1]), per
+
+    for _ in range(args.warmup):
+        step()
+    sync()
+    assert int(status.sum()) == 0, "workload vectors must be inside the supported domain"
+    n0 = ctx.launch_count()
+    ctx.profile_enable(True)
+    clocks = ClockSampler(local)
+    total_ms, wall_ms, per = timed(step, args.steps)
+    clk = clocks.stop()
+    prof, triples = ctx.profile_read()
+    ctx.profile_enable(False)
+    launches = ctx.launch_count() - n0
+    ll_dev = ll.cpu().numpy().copy()
+
+    # e2e: host buffers through the C ABI, copies inside the timed region
+    for _ in range(2):
+        step_e2e()
+    e2e_total, _, _ = timed(step_e2e, args.steps)
+    assert np.array_equal(ll_host, ll_dev), "host-buffer path must reproduce the device-pointer path bit for bit"
+
+    ms_per_step = total_ms / args.steps
+    value = world * B * args.steps / (total_ms * 1e-3)
+    e2e_value = world * B * args.steps / (e2e_total * 1e-3)
+
+    if rank == 0:
+        cells_ms, cells_n = prof["cells"]
+        tri_per_launch = triples / max(cells_n, 1)
+        achieved = FLOP_PER_TRIPLE * tri_per_launch / (cells_ms / max(cells_n, 1) * 1e-3) / 1e12
+        try:
+            peak_dfma = ppm.measure_fp64_peak(local) / 1e12
+        except ppm.PPMError:
+            peak_dfma = None
+        kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
+        roofline = {"bound": "alu", "kernel": "k_cells", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
+                    "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": None,
+                    "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
+                                   "Roofline); MEASURED_PEAKS.json has no FP64 entry",
+                    "peak_measured_dfma_chain": peak_dfma,
+                    "frac_of_measured_dfma_chain": (achieved / peak_dfma) if peak_dfma else None,
+                    "flop_per_unit": FLOP_PER_TRIPLE, "units_per_launch": tri_per_launch,
+                    "kernel_ms_per_launch": cells_ms / max(cells_n, 1),
+                    "kernel_share_of_step": cells_ms / total_ms, "kernel_ms_per_step": kern_ms}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_eval": ms_per_step / B,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": desc, "name": args.workload, "batch_per_gpu": B, "n_fp": ctx.n_fp,
+                           "l2": "flushed before every step (256 MiB write, inside the timed bracket)",
+                           "step": "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params_pinned.numel() * 8),
+                        "d2h_bytes_per_step": int(ll_host.nbytes + st_host.nbytes),
+                        "call": "ppm_loglike_host (host params in, host ln L + status out)"},
+                "gpu_launches": int(launches), "clocks": clk, "wall_ms_per_step": wall_ms / args.steps,
+                "step_ms": [round(x, 3) for x in per], "roofline": roofline, "cpu_baseline": None}
+        if world == 1 and not args.no_cpu_baseline:
+            cb = oracle_sample(conf)
+            line["cpu_baseline"] = {"value": cb["value"], "unit": UNIT, "cores": cb["cores"], "kind": "oracle",
+                                    "sample": cb["sample"]}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -233,3 +233,21 @@ def synthetic_response(energies, n_channel=1500, chan_width=0.01, sigma=0.1, see
     del centres
     return dict(first_chan=first, rsp_band=np.ascontiguousarray(band), tau_ref=tau_ref, n_channel=n_channel,
                 area=area, w=w)
+
+
+def synthetic_counts(n_phase, n_channel, total=1.0e6, bkg_frac=0.05, seed=SEED0 + 7):
+    """Seeded Poisson counts of a smooth pulse x spectrum shape, for throughput runs (bench.py) where
+    the data only have to look like an observation: a 1e6-count exposure with a
+    single-peaked pulse and a thermal-looking channel spectrum, plus a flat background carrying
+    `bkg_frac` of the source counts.  Returns (data[n_phase][n_channel], bkg[n_channel]).
+    Parity tests draw their data from the ORACLE's model instead (tests/test_gpu_parity.py)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    k = np.arange(n_phase, dtype=np.float64) / n_phase
+    Ec = (np.arange(n_channel, dtype=np.float64) + 0.5) * 0.01
+    pulse = 1.0 + 0.35 * np.cos(2.0 * np.pi * (k - 0.2)) + 0.08 * np.cos(4.0 * np.pi * (k - 0.1))
+    spec = Ec ** 2 * np.exp(-Ec / 0.35) * np.exp(-(0.25 / Ec) ** 2.5)
+    m = pulse[:, None] * spec[None, :]
+    m *= total / m.sum()
+    bkg = np.full(n_channel, bkg_frac * total / (n_phase * n_channel))
+    data = rng.poisson(m + bkg[None, :]).astype(np.float64)
+    return data, bkg

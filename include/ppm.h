@@ -141,6 +141,19 @@ int64_t ppm_launch_count(const ppm_ctx* ctx);
 /* Effective n_fp after defaulting. */
 int ppm_n_fp(const ppm_ctx* ctx);
 
+/* Per-kernel device timing, for bench.py's roofline object.  ppm_profile_enable(ctx, 1) resets the
+ * accumulators and from then on brackets every kernel launch of this context with a pair of CUDA
+ * events on the context's stream (no synchronisation is added); ppm_profile_enable(ctx, 0) stops.
+ * ppm_profile_read synchronises the stream and returns, per kernel id, the summed event time in ms
+ * and the number of launches since the last enable:
+ *   PPM_KID_STAR 0, ROWS 1, LOOKUP 2, TEMPLATE 3, SLICE 4, CELLS 5, REDUCE 6, FOLD 7, LOGLIKE 8
+ * ms_host, launches_host: host arrays of PPM_KID_COUNT entries.  *triples_host receives the number
+ * of (active cell, output phase, energy) triples with F_p != 0 that the cell kernel accumulated
+ * since the last enable (the algorithmic unit of DESIGN.md "Roofline"; counted on the device). */
+#define PPM_KID_COUNT 9
+int ppm_profile_enable(ppm_ctx* ctx, int on);
+int ppm_profile_read(ppm_ctx* ctx, double* ms_host, int64_t* launches_host, double* triples_host);
+
 /* Register-resident DFMA chain on every SM: returns the measured FP64 FMA rate in flop/s
  * (2 flop per DFMA) -- the roofline denominator of the cell kernel. */
 int ppm_measure_fp64_peak(int device, double* flops_per_s);

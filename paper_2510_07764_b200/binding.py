@@ -42,6 +42,8 @@ EXPORTS = {
     "ppm_debug_lookup": (C.c_int, [_vp, C.c_int, C.c_int, _dp, C.c_int, _dp, _dp, _dp]),
     "ppm_launch_count": (C.c_int64, [_vp]),
     "ppm_n_fp": (C.c_int, [_vp]),
+    "ppm_profile_enable": (C.c_int, [_vp, C.c_int]),
+    "ppm_profile_read": (C.c_int, [_vp, _dp, C.POINTER(C.c_int64), _dp]),
     "ppm_measure_fp64_peak": (C.c_int, [C.c_int, _dp]),
     "ppm_last_error": (C.c_char_p, []),
 }
@@ -237,6 +239,19 @@ class PPM:
         psi, dpsi, lag = (np.zeros(len(alpha)) for _ in range(3))
         _check(self.lib.ppm_debug_lookup(self._h, b, int(row), _np(alpha), len(alpha), _np(psi), _np(dpsi), _np(lag)))
         return psi, dpsi, lag
+
+    KERNELS = ("star", "rows", "lookup", "template", "slice", "cells", "reduce", "fold", "loglike")
+
+    def profile_enable(self, on=True):
+        _check(self.lib.ppm_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self):
+        """-> (dict kernel -> (ms, launches), triples) since the last profile_enable."""
+        ms = np.zeros(len(self.KERNELS))
+        n = np.zeros(len(self.KERNELS), dtype=np.int64)
+        tr = C.c_double()
+        _check(self.lib.ppm_profile_read(self._h, _np(ms), n.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(tr)))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(self.KERNELS)}, tr.value
 
     def launch_count(self):
         return int(self.lib.ppm_launch_count(self._h))

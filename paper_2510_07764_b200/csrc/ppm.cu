@@ -124,7 +124,34 @@ struct ppm_ctx {
     double *d_params_stage = nullptr, *d_flux_stage = nullptr, *d_ll_stage = nullptr, *d_counts_stage = nullptr;
     int* d_status_stage = nullptr;
     size_t cells_smem = 0;
+    // profiling (ppm_profile_enable / ppm_profile_read): CUDA event pairs around every launch
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev;             // pool, two per recorded launch
+    std::vector<int> prof_kid;                    // kernel id of each recorded launch
+    size_t prof_used = 0;
+    unsigned long long* d_pairs = nullptr;        // (cell, phase) pairs with F_p != 0 walked by k_cells
 };
+
+// kernel ids of ppm_profile_read
+enum { KID_STAR = 0, KID_ROWS, KID_LOOKUP, KID_TEMPLATE, KID_SLICE, KID_CELLS, KID_REDUCE, KID_FOLD, KID_LOGLIKE, KID_N };
+
+static void prof_begin(ppm_ctx* c, int kid)
+{
+    if (!c->prof_on) return;
+    if (c->prof_used + 2 > c->prof_ev.size()) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { c->prof_on = false; return; }
+        c->prof_ev.push_back(a); c->prof_ev.push_back(b);
+    }
+    c->prof_kid.push_back(kid);
+    cudaEventRecord(c->prof_ev[c->prof_used], c->stream);
+}
+static void prof_end(ppm_ctx* c)
+{
+    if (!c->prof_on) return;
+    cudaEventRecord(c->prof_ev[c->prof_used + 1], c->stream);
+    c->prof_used += 2;
+}
 
 extern "C" const char* ppm_last_error(void) { return g_err; }
 
@@ -137,6 +164,8 @@ extern "C" int ppm_destroy(ppm_ctx* c)
                     c->d_tmpl, c->d_slices, c->d_partial, c->d_lgam, c->d_params_stage, c->d_flux_stage,
                     c->d_ll_stage, c->d_counts_stage, c->d_status_stage};
     for (void* p : ptrs) if (p) cudaFree(p);
+    if (c->d_pairs) cudaFree(c->d_pairs);
+    for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     delete c;
     return PPM_OK;
 }
@@ -154,6 +183,8 @@ static int alloc_scratch(ppm_ctx* c)
     if ((rc = dev_alloc(&c->d_tmpl, rows * 4 * (c->n_fp + 1)))) return rc;
     if ((rc = dev_alloc(&c->d_partial, (size_t)c->SB * c->nchunk * g.n_phase * g.n_energy))) return rc;
     if ((rc = dev_alloc(&c->d_lgam, (size_t)1))) return rc;
+    if ((rc = dev_alloc(&c->d_pairs, (size_t)1))) return rc;
+    if (cudaMemsetAsync(c->d_pairs, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return PPM_ERR_CUDA;
     return PPM_OK;
 }
 
@@ -330,25 +361,35 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     G.lookup = c->d_lookup; G.tmpl = c->d_tmpl;
     G.axT = c->d_axT; G.nT = c->nT; G.axg = c->d_axg; G.ng = c->ng;
     const int rows = nb * c->RT;
+    prof_begin(c, KID_STAR);
     k_star<<<(nb + 63) / 64, 64, 0, c->stream>>>(G);
+    prof_end(c);
+    prof_begin(c, KID_ROWS);
     k_rows<<<rows, 128, 0, c->stream>>>(G);
+    prof_end(c);
+    prof_begin(c, KID_LOOKUP);
     k_lookup<<<rows, kNCheb, 0, c->stream>>>(G);
+    prof_end(c);
     const size_t tsm = sizeof(double) * (2 * kNCheb + 4 * (size_t)(c->n_fp + 1));
     if (tsm > 48 * 1024) CK(cudaFuncSetAttribute(k_template, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
+    prof_begin(c, KID_TEMPLATE);
     k_template<<<rows, 128, tsm, c->stream>>>(G);
+    prof_end(c);
     c->launches += 4;
     if (table) {
         SliceArgs S;
         S.spots = c->d_spots; S.rows = c->d_rows; S.values = c->d_values; S.slices = c->d_slices;
         S.n_theta = g.n_theta; S.nT = c->nT; S.ng = c->ng; S.nmu = c->nmu; S.nx = c->nx;
         dim3 sg((c->nmu * c->nx + 255) / 256, rows);
+        prof_begin(c, KID_SLICE);
         k_slice<<<sg, 256, 0, c->stream>>>(S);
+        prof_end(c);
         c->launches += 1;
     }
     CellArgs A;
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
     A.slices = c->d_slices; A.axmu = c->d_axmu; A.ue = c->d_ue; A.le2 = c->d_le2; A.en = c->d_en;
-    A.partial = c->d_partial;
+    A.partial = c->d_partial; A.pairs = c->d_pairs;
     A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;
     A.n_fp = c->n_fp; A.nE = g.n_energy;
@@ -359,11 +400,15 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu + (size_t)c->nw * A.nx);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
+    prof_begin(c, KID_CELLS);
     int rc = table ? dispatch_cells<1>(c, A, grid, c->nw * 32, smem) : dispatch_cells<0>(c, A, grid, c->nw * 32, smem);
+    prof_end(c);
     if (rc) return rc;
     const int n_out = g.n_phase * g.n_energy;
     dim3 rg((n_out + 255) / 256, nb);
+    prof_begin(c, KID_REDUCE);
     k_reduce<<<rg, 256, 0, c->stream>>>(c->d_partial, c->d_stars, c->nchunk, n_out, flux_dev, status_dev);
+    prof_end(c);
     c->launches += 2;
     CK(cudaGetLastError());
     c->last_nb = nb;
@@ -414,7 +459,9 @@ extern "C" int ppm_fold_response(ppm_ctx* c, const double* flux_dev, const doubl
         Fs.params = params_dev + (size_t)b0 * F.P;
         Fs.counts = counts_dev + (size_t)b0 * F.n_phase * F.n_channel;
         dim3 grid((c->n_channel + 127) / 128, c->cfg.n_phase, nb);
+        prof_begin(c, KID_FOLD);
         k_fold<<<grid, 128, smem, c->stream>>>(Fs);
+        prof_end(c);
         c->launches += 1;
     }
     CK(cudaGetLastError());
@@ -432,10 +479,12 @@ extern "C" int ppm_loglike(ppm_ctx* c, const double* counts_dev, int B, const do
     if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
     if (B == 0) return PPM_OK;
     CK(cudaSetDevice(c->cfg.device));
+    prof_begin(c, KID_LOGLIKE);
     k_loglike<<<1, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
                                         nullptr, 1, c->d_lgam);
     k_loglike<<<B, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
                                         c->d_lgam, 0, loglike_dev);
+    prof_end(c);
     c->launches += 2;
     CK(cudaGetLastError());
     return PPM_OK;
@@ -602,6 +651,36 @@ extern "C" int ppm_debug_lookup(ppm_ctx* c, int b, int row, const double* alpha,
     if (e == cudaSuccess) e = cudaMemcpy(lag, d + 3 * n, sizeof(double) * n, cudaMemcpyDeviceToHost);
     cudaFree(d);
     if (e != cudaSuccess) { set_err("ppm_debug_lookup: %s", cudaGetErrorString(e)); return PPM_ERR_CUDA; }
+    return PPM_OK;
+}
+
+extern "C" int ppm_profile_enable(ppm_ctx* c, int on)
+{
+    ARG(c, "null context");
+    CK(cudaSetDevice(c->cfg.device));
+    CK(cudaStreamSynchronize(c->stream));
+    c->prof_on = on != 0;
+    c->prof_used = 0;
+    c->prof_kid.clear();
+    CK(cudaMemsetAsync(c->d_pairs, 0, sizeof(unsigned long long), c->stream));
+    return PPM_OK;
+}
+
+extern "C" int ppm_profile_read(ppm_ctx* c, double* ms, int64_t* launches, double* triples)
+{
+    ARG(c && ms && launches && triples, "null pointer");
+    CK(cudaSetDevice(c->cfg.device));
+    CK(cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < KID_N; ++i) { ms[i] = 0.0; launches[i] = 0; }
+    for (size_t i = 0; i < c->prof_kid.size() && 2 * i + 1 < c->prof_used; ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+        ms[c->prof_kid[i]] += (double)t;
+        launches[c->prof_kid[i]] += (c->prof_kid[i] == KID_LOGLIKE) ? 2 : 1;
+    }
+    unsigned long long pairs = 0;
+    CK(cudaMemcpy(&pairs, c->d_pairs, sizeof(pairs), cudaMemcpyDeviceToHost));
+    *triples = (double)pairs * (double)c->cfg.n_energy;
     return PPM_OK;
 }
 

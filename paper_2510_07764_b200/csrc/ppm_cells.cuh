@@ -17,6 +17,7 @@ struct CellArgs {
     const double* le2;       // [nE]: -log2(E_e)
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
+    unsigned long long* pairs;   // counter: (cell, phase) pairs with F_p != 0 (energy tile 0 only)
     double x0_over_h, inv_h;
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
@@ -134,6 +135,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
     const StarD& st = A.stars[b];
     const double phi_off = st.phi_off;
     const double phi_out = (double)k / A.n_phase;                               // reading R3
+    unsigned npairs = 0;
 
     for (int ri = 0; ri < A.rows_per_chunk; ++ri) {
         const int rl = chunk + ri * A.nchunk;                                   // strided chunks balance row sizes
@@ -199,6 +201,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                 }
             }
             unsigned todo = __ballot_sync(0xffffffffu, Fp != 0.0);
+            npairs += __popc(todo);
             // ---- step B: walk the valid pairs ----
             while (todo) {
                 const int j = __ffs(todo) - 1;
@@ -268,6 +271,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
             }
         }
     }
+    if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
     if (kvalid) {
         double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
 #pragma unroll
