@@ -46,12 +46,14 @@ METRIC = "pulse-profile evaluations per second"
 UNIT = "evals/s"
 
 
-def workload(name, batch, rank):
+def workload(name, batch, rank, world=1):
     """-> (conf dict with `batch` parameter vectors for this rank, description)."""
+    from paper_2510_07764_b200.shard import shard_slice
     if name in ("C5", "T"):
         B = 1 if name == "T" else batch
-        conf = gen.config_c5(n_vec=B * (rank + 1))
-        conf["params"] = np.ascontiguousarray(conf["params"][B * rank:B * (rank + 1)])
+        lo, hi = shard_slice(B * world, rank, world)              # weak scaling: B vectors of C5 per rank
+        conf = gen.config_c5(n_vec=B * world)
+        conf["params"] = np.ascontiguousarray(conf["params"][lo:hi])
         desc = ("BASELINE.json configs[4] (C5 batched likelihood): %d seeded prior vectors per GPU, each 2 spots x "
                 "256x256 cells, 128 phases x 300 energies 0.2-12 keV, mixed-order interpolation on the synthetic "
                 "35x11x67x166 table, banded fold 300 -> 1500 channels, Poisson ln L" % B)
@@ -185,6 +187,7 @@ def main():
 
     import torch
     import paper_2510_07764_b200 as ppm
+    from paper_2510_07764_b200.shard import max_over_ranks
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the PPM hot path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -194,7 +197,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    conf, desc = workload(args.workload, args.batch, rank)
+    conf, desc = workload(args.workload, args.batch, rank, world)
     cfg, E = conf["cfg"], conf["energies"]
     B = conf["params"].shape[0]
     ctx = ppm.PPM(cfg, E, max_batch=B, device=local)
@@ -244,10 +247,8 @@ def main():
         wall = time.perf_counter() - t0
         per = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(k)]
         total = ev[0].elapsed_time(ev[2 * k - 1])
-        t = torch.tensor([total, wall * 1e3], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t[0]), float(t[1]), per
+        t = max_over_ranks([total, wall * 1e3], device=dev)
+        return t[0], t[1], per
 
     for _ in range(args.warmup):
         step()
