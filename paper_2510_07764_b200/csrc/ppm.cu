@@ -100,7 +100,7 @@ struct ppm_ctx {
     ppm_config cfg;
     cudaStream_t stream = nullptr;
     int P = 0, RT = 0, n_fp = 0, SB = 1;          // params per vector, rows per vector, sub-batch size
-    int nchunk = 1, rows_per_chunk = 1, nw = 1, npg = 1, epl = 1, n_etile = 1;
+    int nchunk = 1, rows_per_chunk = 1, nw = 1, npg = 1, epl = 1, n_etile = 1, wmax = 0;
     int64_t launches = 0;
     int last_nb = 0;
     // energy grid
@@ -258,6 +258,7 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
 {
     ARG(c && logT && logg && mu && logx && values, "null pointer");
     ARG(nT >= 4 && ng >= 4 && nmu >= 4 && nx >= 4, "every table axis needs >= 4 nodes");
+    ARG(nmu <= 128 && nx <= 256, "the cell kernel packs stencil indices: nmu <= 128 and nx <= 256");
     const double* axs[4] = {logT, logg, mu, logx};
     const int ns[4] = {nT, ng, nmu, nx};
     for (int a = 0; a < 4; ++a)
@@ -282,6 +283,12 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     std::vector<double> ue(c->cfg.n_energy);
     for (int e = 0; e < c->cfg.n_energy; ++e) ue[e] = std::log10(c->h_en[e]) / h;
     CK(cudaMemcpyAsync(c->d_ue, ue.data(), sizeof(double) * ue.size(), cudaMemcpyHostToDevice, c->stream));
+    // most logx intervals the energies of one tile can touch for one (cell, phase) pair
+    c->wmax = 1;
+    for (int t = 0; t < c->n_etile; ++t) {
+        const int ea = t * 32 * c->epl, eb = std::min(c->cfg.n_energy, ea + 32 * c->epl) - 1;
+        c->wmax = std::max(c->wmax, std::min(nx - 1, (int)std::floor(ue[eb] - ue[ea]) + 3));
+    }
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;
@@ -397,7 +404,9 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_MIXED ? 1 : 0;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
-    const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu + (size_t)c->nw * A.nx);
+    A.wmax = table ? c->wmax : 0;
+    const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu +
+                                          (size_t)c->nw * (A.nx + 4 * (size_t)A.wmax));
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
     prof_begin(c, KID_CELLS);

@@ -22,6 +22,7 @@ struct CellArgs {
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
     int nchunk, rows_per_chunk, nw, n_etile;
+    int wmax;                // table path: most logx intervals one (pair, energy tile) can touch
 };
 
 // ---- K4: collapse the 4-D table to the row's (mu x logx) slice: T is per spot, g per row -------
@@ -54,36 +55,27 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
     A.slices[(size_t)rid * plane + i] = v;
 }
 
-// 2^f on [-0.5, 0.5]: Taylor series of exp(f ln 2) to degree 12 (truncation < 2e-16 relative)
-__device__ __forceinline__ double exp2_poly(double f)
-{
-    // c_n = (ln 2)^n / n!
-    double p = 2.567843599348820514199e-11;                 // n = 12
-    p = fma(p, f, 4.445538271870811497596e-10);             // 11
-    p = fma(p, f, 7.054911620801123329875e-9);              // 10
-    p = fma(p, f, 1.017808600923969972749e-7);              // 9
-    p = fma(p, f, 1.321548679014430948840e-6);              // 8
-    p = fma(p, f, 1.525273380405984028003e-5);              // 7
-    p = fma(p, f, 1.540353039338160995443e-4);              // 6
-    p = fma(p, f, 1.333355814642844342341e-3);              // 5
-    p = fma(p, f, 9.618129107628477161980e-3);              // 4
-    p = fma(p, f, 5.550410866482157995314e-2);              // 3
-    p = fma(p, f, 2.402265069591007123336e-1);              // 2
-    p = fma(p, f, 6.931471805599453094172e-1);              // 1
-    p = fma(p, f, 1.0);
-    return p;
-}
-
-// 2^y for any y: round, polynomial, exponent add (integer pipe).  y < -1000 -> 0.
-__device__ __forceinline__ double exp2_fast(double y)
+// 2^y for the table path: y = n + f, n = round(y) through the 1.5*2^52 constant, |f| <= 1/2;
+// 2^f by a degree-10 polynomial (Chebyshev-node fit on [-1/2, 1/2]; max relative error 4.3e-16 in double
+// arithmetic), 2^n by an integer add into the exponent field.  y < -1000 -> 0.
+__device__ __forceinline__ double exp2_p10(double y)
 {
     const double r = y + kMagic;
     const int n = __double2loint(r);
     const double f = y - (r - kMagic);
-    const double p = exp2_poly(f);
+    double p = 7.072585949269223e-09;
+    p = fma(p, f, 1.0208690299958306e-07);
+    p = fma(p, f, 1.321544258792169e-06);
+    p = fma(p, f, 1.5252657260200837e-05);
+    p = fma(p, f, 0.0001540353044173605);
+    p = fma(p, f, 0.0013333558230164974);
+    p = fma(p, f, 0.009618129107606888);
+    p = fma(p, f, 0.05550410866444772);
+    p = fma(p, f, 0.24022650695910097);
+    p = fma(p, f, 0.69314718055995);
+    p = fma(p, f, 1.0);
     const int hi = __double2hiint(p) + n * 1048576;
-    const int lo = __double2loint(p);
-    return (n < -1000) ? 0.0 : __hiloint2double(hi, lo);
+    return (n < -1000) ? 0.0 : __hiloint2double(hi, __double2loint(p));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -91,11 +83,17 @@ __device__ __forceinline__ double exp2_fast(double y)
 // tile); warp w owns output phase k and the 32*EPL energies of the tile (lane owns energies
 // e0+lane+32 i): the (k, e) accumulators live in registers for the whole chunk -- output-stationary,
 // no atomics.  Per row the (mu x logx) slice and the ring template sit in shared memory.  Lanes first
-// prepare 32 (cell, k) pairs in parallel (Eq 45-46, mu stencil), then the warp walks the valid pairs:
-// contract the mu stencil into a 1-D vector over logx (shared by all energies of the pair), then each
-// lane interpolates in logx and accumulates F_p I / E (Eq 47) as one exp2.
+// prepare 32 (cell, k) pairs in parallel (Eq 45-46, mu stencil, the window of logx intervals the pair's
+// energies fall in), then the warp walks the pairs with F_p != 0.  Per pair (work shared by all its
+// energies): contract the mu stencil into node values over the window, then turn every interval of
+// the window into the monomial coefficients k0..k3 of its interpolating polynomial in
+// tau = (x - x_mid)/h (cubic Lagrange on the 4 surrounding nodes; linear / shifted stencil in the edge
+// intervals per strategy), pre-scaled by log2(10) and with log2(F_p T^3) added to k0.  Per triple:
+// interval index + tau (4 DADD), Horner (3 DFMA), exp2_p10 (3 DADD + 10 DFMA), accumulate (1 DADD).
+// The division by E_e of Eq 47 is the same for every term of a bin and is applied once in the epilogue.
 // MODE 0: closed-form isotropic blackbody (Eq C.5); MODE 1: table.
 // ------------------------------------------------------------------------------------------------
+
 template <int EPL, int MODE>
 __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
 {
@@ -107,20 +105,27 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
     const bool kvalid = k < A.n_phase;
     const int e0 = et * 32 * EPL;
     const int n1 = A.n_fp + 1;
-    const int plane = (MODE == 1) ? A.nmu * A.nx : 0;
-    double* S = sm;                                  // [nmu][nx]
-    double* T = sm + plane;                          // F, z, phi_o, mu: [4][n1]
-    double* MUAX = T + 4 * n1;                       // [nmu]
-    double* CV = MUAX + ((MODE == 1) ? A.nmu : 0) + (size_t)w * A.nx;   // per-warp contracted vector [nx]
+    const int nx = A.nx;
+    const int plane = (MODE == 1) ? A.nmu * nx : 0;
+    // shared layout: per warp KA [wmax] (k0, k1), KB [wmax] (k2, k3) as double2 (16-byte aligned; two arrays so that
+    // lanes writing / reading consecutive intervals touch consecutive 16-byte words: no bank conflicts)
+    // | S [nmu][nx] | T [4][n1] | MUAX [nmu] | CV per warp [nx]
+    const int kc_len = (MODE == 1) ? 4 * A.wmax : 0;
+    double* KCall = sm;
+    double* S = KCall + (size_t)A.nw * kc_len;
+    double* T = S + plane;
+    double* MUAX = T + 4 * n1;
+    double* CV = MUAX + ((MODE == 1) ? A.nmu : 0) + (size_t)w * nx;
+    double2* KA = reinterpret_cast<double2*>(KCall + (size_t)w * kc_len);
+    double2* KB = KA + A.wmax;
 
-    double ue[EPL], c2[EPL], acc[EPL];
+    double ue[EPL], c2[(MODE == 0) ? EPL : 1], acc[EPL];
 #pragma unroll
     for (int i = 0; i < EPL; ++i) {
         const int e = e0 + lane + 32 * i;
         const bool ok = e < A.nE;
         if (MODE == 1) {
             ue[i] = A.ue[ok ? e : A.nE - 1];
-            c2[i] = ok ? A.le2[e] : -5000.0;
         } else {
             ue[i] = ok ? A.en[e] : 1.0;              // E_e
             c2[i] = ok ? 1.0 : 0.0;
@@ -147,7 +152,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
         const SpotD& sp = A.spots[rid / A.n_theta];
         __syncthreads();
         {   // stage slice + template (16-byte loads)
-            if ((plane & 1) == 0) {
+            if ((plane & 1) == 0 && ((A.nw * kc_len) & 1) == 0) {
                 const double2* src = reinterpret_cast<const double2*>(A.slices + (size_t)rid * plane);
                 double2* dst = reinterpret_cast<double2*>(S);
                 for (int i = threadIdx.x; i < plane / 2; i += blockDim.x) dst[i] = src[i];
@@ -169,9 +174,9 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
         for (int base = 0; base < nact; base += 32) {
             // ---- step A: lane <-> cell; Eq 45-46 and the per-pair constants ----
             const int idx = base + lane;
-            double Fp = 0.0, pa = 0.0, pb = 0.0;      // MODE 1: pa = uz, pb = lf;  MODE 0: pa = z_p, pb = F_p z_p^3 K
+            double Fp = 0.0, pa = 0.0, pb = 0.0;      // MODE 1: pa = uz, pb = log2(F_p T^3);  MODE 0: pa = z_p / kT, pb = F_p z_p^3 K
             double w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0;
-            int mb = 0;
+            int info = 0;                             // MODE 1: mu stencil base | jlo << 7 | jhi << 15 | fast << 23
             if (idx < nact) {
                 const int m = cl[idx];
                 const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
@@ -189,11 +194,20 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                 const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
                 if (Fp != 0.0) {
                     if (MODE == 1) {
-                        pa = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h - 0.5;   // u - 0.5 = (x - x0)/h - 0.5, less the energy part
+                        pa = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h - 0.5;   // (x - x0)/h - 0.5, less the energy part
                         pb = log2(Fp) + sp.log2T3;
                         double ww[4];
+                        int mb;
                         axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
-                        w0 = ww[0]; w1 = ww[1]; w2 = ww[2]; w3 = ww[3];
+                        w0 = ww[0] * kLog2_10; w1 = ww[1] * kLog2_10; w2 = ww[2] * kLog2_10; w3 = ww[3] * kLog2_10;
+                        // window of logx intervals touched by this pair's energies, found with the very arithmetic
+                        // the energy loop uses (monotone in e, so first / last energy bound every index)
+                        const double hi_c = (double)nx - 1.5;
+                        const double ua = pa + ue_first, ub = pa + ue_last;
+                        const int fast = (ua >= -0.5) && (ub < hi_c);
+                        const int jlo = imin_(__double2loint(fmin(fmax(ua, -0.5), hi_c) + kMagic), nx - 2);
+                        const int jhi = imin_(__double2loint(fmin(fmax(ub, -0.5), hi_c) + kMagic), nx - 2);
+                        info = mb | (jlo << 7) | (jhi << 15) | (fast << 23);
                     } else {
                         pa = zp / sp.kT;
                         pb = Fp * (2.0 / (kH_keV_s * kH_keV_s * kH_keV_s * kC_cm_s * kC_cm_s)) * zp * zp * zp;
@@ -208,7 +222,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                 todo &= todo - 1;
                 const double qa = __shfl_sync(0xffffffffu, pa, j);
                 const double qb = __shfl_sync(0xffffffffu, pb, j);
-                if (MODE == 0) {
+                if constexpr (MODE == 0) {
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
                         const double E = ue[i];
@@ -220,17 +234,47 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                 const double v1 = __shfl_sync(0xffffffffu, w1, j);
                 const double v2 = __shfl_sync(0xffffffffu, w2, j);
                 const double v3 = __shfl_sync(0xffffffffu, w3, j);
-                const int sb = __shfl_sync(0xffffffffu, mb, j);
-                // column range of logx touched by this pair's energies
-                const double ulo = qa + ue_first + 0.5, uhi = qa + ue_last + 0.5;
-                const bool fast = (ulo >= 1.5) && (uhi < (double)A.nx - 2.5);
-                const int jlo = imin_(imax_((int)floor(fmin(fmax(ulo, 0.0), (double)A.nx)) - 2, 0), A.nx - 4);
-                const int jhi = imin_(imax_((int)floor(fmin(fmax(uhi, 0.0), (double)A.nx)) + 2, 3), A.nx - 1);
-                const double* s0p = S + (size_t)sb * A.nx;
+                const int inf = __shfl_sync(0xffffffffu, info, j);
+                const int sb = inf & 127, jlo = (inf >> 7) & 255, jhi = (inf >> 15) & 255;
+                const bool fast = (inf >> 23) & 1;
+                // node values log2(10) * sum_mu w_mu S[mu][c] on the nodes the window's stencils touch
+                const int nlo = imin_(imax_(jlo - 1, 0), nx - 4);
+                const int nhi = imin_(imax_(jhi + 2, nlo + 3), nx - 1);
                 __syncwarp();
-                for (int c = jlo + lane; c <= jhi; c += 32)
-                    CV[c] = fma(v3, s0p[3 * A.nx + c], fma(v2, s0p[2 * A.nx + c], fma(v1, s0p[A.nx + c], v0 * s0p[c])));
+                {
+                    const double* sp0 = S + sb * nx + nlo + lane;
+                    double* cv = CV + nlo + lane;
+                    for (int c = nlo + lane; c <= nhi; c += 32, sp0 += 32, cv += 32)
+                        *cv = fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
+                }
                 __syncwarp();
+                // per interval c in [jlo, jhi]: monomial coefficients in tau (offset from the interval midpoint, in units of h)
+                for (int c = jlo + lane; c <= jhi; c += 32) {
+                    const int s = imin_(imax_(c - 1, 0), nx - 4);
+                    const double* cvs = CV + s;
+                    const double c0 = cvs[0], c1 = cvs[1], c2v = cvs[2], c3 = cvs[3];
+                    const double s03 = c0 + c3, s12 = c1 + c2v, d30 = c3 - c0, d21 = c2v - c1;
+                    double k0 = fma(s03, -0.0625, s12 * 0.5625);
+                    double k1 = fma(d30, -1.0 / 24.0, d21 * 1.125);
+                    double k2 = (s03 - s12) * 0.25;
+                    double k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
+                    if (s != c - 1) {                                           // first / last interval of the axis
+                        if (A.x_linedge) {                                      // strategy d: linear
+                            const double a = CV[c], bb = CV[c + 1];
+                            k0 = 0.5 * (a + bb); k1 = bb - a; k2 = 0.0; k3 = 0.0;
+                        } else {                                                // strategy a: shifted stencil, Taylor shift by d
+                            const double d = (double)(c - 1 - s);
+                            k0 = fma(d, fma(d, fma(d, k3, k2), k1), k0);
+                            k1 = fma(d, fma(3.0 * d, k3, 2.0 * k2), k1);
+                            k2 = fma(3.0 * d, k3, k2);
+                        }
+                    }
+                    KA[c - jlo] = make_double2(k0 + qb, k1);
+                    KB[c - jlo] = make_double2(k2, k3);
+                }
+                __syncwarp();
+                const double2* KAj = KA - jlo;
+                const double2* KBj = KB - jlo;
                 if (fast) {
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
@@ -238,34 +282,20 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                         const double r = uu + kMagic;
                         const int ii = __double2loint(r);                       // interval index, x in [x_ii, x_ii+1]
                         const double tau = uu - (r - kMagic);                   // offset from the interval midpoint
-                        const double c0 = CV[ii - 1], c1 = CV[ii], c2v = CV[ii + 1], c3 = CV[ii + 2];
-                        // cubic Lagrange on nodes at -1.5, -0.5, 0.5, 1.5 (uniform logx axis)
-                        const double a = tau * tau;
-                        const double A6 = fma(a, 1.0 / 6.0, -1.0 / 24.0);
-                        const double B2 = fma(a, 0.5, -1.125);
-                        const double e1 = fma(tau, c3 - c0, 1.5 * (c3 + c0));
-                        const double e2 = fma(tau, c1 - c2v, -0.5 * (c1 + c2v));
-                        const double p = fma(A6, e1, B2 * e2);
-                        acc[i] += exp2_fast(fma(p, kLog2_10, qb) + c2[i]);      // F_p T^3 10^v / E
+                        const double2 ka = KAj[ii], kb = KBj[ii];
+                        acc[i] += exp2_p10(fma(fma(fma(kb.y, tau, kb.x), tau, ka.y), tau, ka.x));
                     }
                 } else {
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
-                        double uq = qa + ue[i] + 0.5;                           // (x - x0)/h, clamped (reading R13b)
-                        uq = fmin(fmax(uq, 0.0), (double)(A.nx - 1));
-                        const int ii = imin_((int)uq, A.nx - 2);
-                        double p;
-                        if (A.x_linedge && (ii == 0 || ii == A.nx - 2)) {      // strategy d: linear edge intervals
-                            const double t = uq - (double)ii;
-                            p = (1.0 - t) * CV[ii] + t * CV[ii + 1];
-                        } else {                                                // interior, or shifted stencil (strategy a)
-                            const int s = imin_(imax_(ii - 1, 0), A.nx - 4);
-                            const double g = uq - (double)s;                    // in [0, 3]
-                            const double g1 = g - 1.0, g2 = g - 2.0, g3 = g - 3.0;
-                            p = (-1.0 / 6.0) * (g1 * g2 * g3) * CV[s] + 0.5 * (g * g2 * g3) * CV[s + 1]
-                              - 0.5 * (g * g1 * g3) * CV[s + 2] + (1.0 / 6.0) * (g * g1 * g2) * CV[s + 3];
-                        }
-                        acc[i] += exp2_fast(fma(p, kLog2_10, qb) + c2[i]);
+                        // clamp (x - x0)/h to [0, nx-1] (reading R13b); a tie at the upper end may round to interval nx-1
+                        const double uu = fmin(fmax(qa + ue[i], -0.5), (double)nx - 1.5);
+                        const double r = uu + kMagic;
+                        int ii = __double2loint(r);
+                        double tau = uu - (r - kMagic);
+                        if (ii > nx - 2) { ii = nx - 2; tau += 1.0; }
+                        const double2 ka = KAj[ii], kb = KBj[ii];
+                        acc[i] += exp2_p10(fma(fma(fma(kb.y, tau, kb.x), tau, ka.y), tau, ka.x));
                     }
                 }
             }
@@ -277,7 +307,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
             const int e = e0 + lane + 32 * i;
-            if (e < A.nE) out[e] = acc[i];
+            if (e < A.nE) out[e] = (MODE == 1) ? acc[i] / A.en[e] : acc[i];    // the 1/E_e of Eq 47
         }
     }
 }
