@@ -105,6 +105,8 @@ struct ppm_ctx {
     int last_nb = 0;
     // energy grid
     double *d_en = nullptr, *d_ue = nullptr, *d_le2 = nullptr;
+    long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
+    int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
     std::vector<double> h_en;
     // atmosphere
     bool have_atm = false;
@@ -159,7 +161,7 @@ extern "C" int ppm_destroy(ppm_ctx* c)
 {
     if (!c) return PPM_OK;
     cudaSetDevice(c->cfg.device);
-    void* ptrs[] = {c->d_en, c->d_ue, c->d_le2, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
+    void* ptrs[] = {c->d_en, c->d_ue, c->d_le2, c->d_uef, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
                     c->d_ehi, c->d_band, c->d_tau, c->d_stars, c->d_spots, c->d_rows, c->d_cells, c->d_lookup,
                     c->d_tmpl, c->d_slices, c->d_partial, c->d_lgam, c->d_params_stage, c->d_flux_stage,
                     c->d_ll_stage, c->d_counts_stage, c->d_status_stage};
@@ -214,12 +216,18 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     c->n_fp = cfg->n_fp > 0 ? cfg->n_fp : std::max(192, 2 * cfg->n_phase);           // reading R2
     c->h_en.assign(energies, energies + cfg->n_energy);
     // launch geometry of the cell kernel
-    c->nw = std::min(16, cfg->n_phase);
+    // experiment knobs (to be frozen): PPM_CELLS_NW warps per block (16 or 32), PPM_CELLS_EPL energies per lane
+    const char* env_nw = getenv("PPM_CELLS_NW");
+    const char* env_epl = getenv("PPM_CELLS_EPL");
+    const int nw_max = (env_nw && cfg->emission != PPM_EMISSION_BLACKBODY) ? atoi(env_nw) : 16;
+    c->nw = std::min(nw_max, cfg->n_phase);
     c->npg = (cfg->n_phase + c->nw - 1) / c->nw;
     const int need = (cfg->n_energy + 31) / 32;
-    const int epls[] = {1, 2, 4, 8, 10};
+    const int epls[] = {1, 2, 4, 5, 8, 10};
     c->epl = 10;
     for (int v : epls) if (v >= need) { c->epl = v; break; }
+    if (env_epl && cfg->emission != PPM_EMISSION_BLACKBODY) c->epl = atoi(env_epl);
+    if (c->nw > 16 && c->epl > 5) c->epl = 5;
     c->n_etile = (cfg->n_energy + 32 * c->epl - 1) / (32 * c->epl);
     const double per_row = (double)cfg->n_phase * cfg->n_energy * 8.0;
     c->rows_per_chunk = 1;
@@ -235,6 +243,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     if (rc) { ppm_destroy(c); return rc; }
     // energy-derived constants: filled here for blackbody; refreshed by ppm_load_atmosphere (needs h)
     if ((rc = dev_alloc(&c->d_en, (size_t)cfg->n_energy)) || (rc = dev_alloc(&c->d_ue, (size_t)cfg->n_energy)) ||
+        (rc = dev_alloc(&c->d_uef, (size_t)cfg->n_energy)) ||
         (rc = dev_alloc(&c->d_le2, (size_t)cfg->n_energy))) { ppm_destroy(c); return rc; }
     std::vector<double> le2(cfg->n_energy);
     for (int e = 0; e < cfg->n_energy; ++e) le2[e] = -std::log2(energies[e]);
@@ -258,7 +267,7 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
 {
     ARG(c && logT && logg && mu && logx && values, "null pointer");
     ARG(nT >= 4 && ng >= 4 && nmu >= 4 && nx >= 4, "every table axis needs >= 4 nodes");
-    ARG(nmu <= 128 && nx <= 256, "the cell kernel packs stencil indices: nmu <= 128 and nx <= 256");
+    ARG(nx <= 256 && (size_t)nmu * nx <= 32767, "the cell kernel packs stencil indices: nx <= 256 and nmu * nx <= 32767");
     const double* axs[4] = {logT, logg, mu, logx};
     const int ns[4] = {nT, ng, nmu, nx};
     for (int a = 0; a < 4; ++a)
@@ -283,12 +292,21 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     std::vector<double> ue(c->cfg.n_energy);
     for (int e = 0; e < c->cfg.n_energy; ++e) ue[e] = std::log10(c->h_en[e]) / h;
     CK(cudaMemcpyAsync(c->d_ue, ue.data(), sizeof(double) * ue.size(), cudaMemcpyHostToDevice, c->stream));
+    std::vector<long long> uef(c->cfg.n_energy);
+    for (int e = 0; e < c->cfg.n_energy; ++e) {
+        ARG(std::fabs(ue[e]) < 1000.0, "energies are too far outside the table's log10(E/kT) range");
+        uef[e] = llrintl((long double)ue[e] * 4503599627370496.0L);
+    }
+    CK(cudaMemcpyAsync(c->d_uef, uef.data(), sizeof(long long) * uef.size(), cudaMemcpyHostToDevice, c->stream));
     // most logx intervals the energies of one tile can touch for one (cell, phase) pair
     c->wmax = 1;
     for (int t = 0; t < c->n_etile; ++t) {
         const int ea = t * 32 * c->epl, eb = std::min(c->cfg.n_energy, ea + 32 * c->epl) - 1;
         c->wmax = std::max(c->wmax, std::min(nx - 1, (int)std::floor(ue[eb] - ue[ea]) + 3));
     }
+    c->npl = 1;
+    while (32 * c->npl - 3 < c->wmax) c->npl += 2;                 // odd: conflict-free strided shared-memory accesses
+    if (getenv("PPM_CELLS_NPL2") && 61 >= c->wmax) c->npl = 2;
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;
@@ -333,27 +351,54 @@ extern "C" int ppm_set_response(ppm_ctx* c, int n_channel, int band_w, const int
 // ------------------------------------------------------------------------------------------------
 // evaluation
 // ------------------------------------------------------------------------------------------------
-template <int EPL, int MODE>
-static int launch_cells(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+template <typename K>
+static int launch_cells(ppm_ctx* c, K kernel, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
-    static thread_local size_t configured = 0;
-    if (smem > configured) {
-        CK(cudaFuncSetAttribute(k_cells<EPL, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
-    k_cells<EPL, MODE><<<grid, threads, smem, c->stream>>>(a);
+    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kernel<<<grid, threads, smem, c->stream>>>(a);
     return PPM_OK;
 }
 
-template <int MODE>
-static int dispatch_cells(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+template <int EPL, int NT>
+static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
+    switch (c->npl) {
+    case 1:  return launch_cells(c, k_cells_tab<EPL, 1, NT>, a, grid, threads, smem);
+    case 2:  return launch_cells(c, k_cells_tab<EPL, 2, NT>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_tab<EPL, 3, NT>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_tab<EPL, 5, NT>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_tab<EPL, 7, NT>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_tab<EPL, 9, NT>, a, grid, threads, smem);
+    }
+}
+
+static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    if (table && threads > 512) {
+        switch (c->epl) {
+        case 1:  return dispatch_cells_tab<1, 1024>(c, a, grid, threads, smem);
+        case 2:  return dispatch_cells_tab<2, 1024>(c, a, grid, threads, smem);
+        case 4:  return dispatch_cells_tab<4, 1024>(c, a, grid, threads, smem);
+        default: return dispatch_cells_tab<5, 1024>(c, a, grid, threads, smem);
+        }
+    }
+    if (table) {
+        switch (c->epl) {
+        case 1:  return dispatch_cells_tab<1, 512>(c, a, grid, threads, smem);
+        case 2:  return dispatch_cells_tab<2, 512>(c, a, grid, threads, smem);
+        case 4:  return dispatch_cells_tab<4, 512>(c, a, grid, threads, smem);
+        case 5:  return dispatch_cells_tab<5, 512>(c, a, grid, threads, smem);
+        case 8:  return dispatch_cells_tab<8, 512>(c, a, grid, threads, smem);
+        default: return dispatch_cells_tab<10, 512>(c, a, grid, threads, smem);
+        }
+    }
     switch (c->epl) {
-    case 1:  return launch_cells<1, MODE>(c, a, grid, threads, smem);
-    case 2:  return launch_cells<2, MODE>(c, a, grid, threads, smem);
-    case 4:  return launch_cells<4, MODE>(c, a, grid, threads, smem);
-    case 8:  return launch_cells<8, MODE>(c, a, grid, threads, smem);
-    default: return launch_cells<10, MODE>(c, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells<1, 0>, a, grid, threads, smem);
+    case 2:  return launch_cells(c, k_cells<2, 0>, a, grid, threads, smem);
+    case 4:  return launch_cells(c, k_cells<4, 0>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells<5, 0>, a, grid, threads, smem);
+    case 8:  return launch_cells(c, k_cells<8, 0>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells<10, 0>, a, grid, threads, smem);
     }
 }
 
@@ -395,7 +440,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     }
     CellArgs A;
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
-    A.slices = c->d_slices; A.axmu = c->d_axmu; A.ue = c->d_ue; A.le2 = c->d_le2; A.en = c->d_en;
+    A.slices = c->d_slices; A.axmu = c->d_axmu; A.ue = c->d_ue; A.uef = c->d_uef; A.le2 = c->d_le2; A.en = c->d_en;
     A.partial = c->d_partial; A.pairs = c->d_pairs;
     A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;
@@ -406,11 +451,11 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
     A.wmax = table ? c->wmax : 0;
     const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu +
-                                          (size_t)c->nw * (A.nx + 4 * (size_t)A.wmax));
+                                          (table ? (size_t)c->nw * (4 * 32 * c->npl + 3 * 64 + 16) : 0));
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
     prof_begin(c, KID_CELLS);
-    int rc = table ? dispatch_cells<1>(c, A, grid, c->nw * 32, smem) : dispatch_cells<0>(c, A, grid, c->nw * 32, smem);
+    int rc = dispatch_cells(c, table, A, grid, c->nw * 32, smem);
     prof_end(c);
     if (rc) return rc;
     const int n_out = g.n_phase * g.n_energy;

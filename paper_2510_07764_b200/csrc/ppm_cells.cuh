@@ -14,6 +14,7 @@ struct CellArgs {
     const double* slices;    // [rows][nmu][nx]  (table emission)
     const double* axmu;      // [nmu]
     const double* ue;        // [nE]: log10(E_e) / h   (h = logx spacing)
+    const long long* uef;    // [nE]: round(ue * 2^52): the same in fixed point (units of 2^-52 intervals)
     const double* le2;       // [nE]: -log2(E_e)
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
@@ -58,6 +59,22 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
 // 2^y for the table path: y = n + f, n = round(y) through the 1.5*2^52 constant, |f| <= 1/2;
 // 2^f by a degree-10 polynomial (Chebyshev-node fit on [-1/2, 1/2]; max relative error 4.3e-16 in double
 // arithmetic), 2^n by an integer add into the exponent field.  y < -1000 -> 0.
+__device__ __forceinline__ double exp2_frac_scaled(double f, int n)      // 2^f * 2^n, |f| <= 1/2, no range check
+{
+    double p = 7.072585949269223e-09;
+    p = fma(p, f, 1.0208690299958306e-07);
+    p = fma(p, f, 1.321544258792169e-06);
+    p = fma(p, f, 1.5252657260200837e-05);
+    p = fma(p, f, 0.0001540353044173605);
+    p = fma(p, f, 0.0013333558230164974);
+    p = fma(p, f, 0.009618129107606888);
+    p = fma(p, f, 0.05550410866444772);
+    p = fma(p, f, 0.24022650695910097);
+    p = fma(p, f, 0.69314718055995);
+    p = fma(p, f, 1.0);
+    return __hiloint2double(__double2hiint(p) + n * 1048576, __double2loint(p));
+}
+
 __device__ __forceinline__ double exp2_p10(double y)
 {
     const double r = y + kMagic;
@@ -308,6 +325,281 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
         for (int i = 0; i < EPL; ++i) {
             const int e = e0 + lane + 32 * i;
             if (e < A.nE) out[e] = (MODE == 1) ? acc[i] / A.en[e] : acc[i];    // the 1/E_e of Eq 47
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K5t: the table-emission cell kernel (the dominant kernel of the path).  Same block / warp / lane
+// ownership as k_cells above (output-stationary accumulators, no atomics); what differs is how a
+// (cell, phase) pair is turned into its energies' terms:
+//  * logx coordinate in fixed point.  u = (log10(z_p E_e / kT) - x0)/h = u_pair + u_e is carried as a
+//    64-bit integer in units of 2^-52 intervals: s = q_pair + uef[e] (two integer adds).  The interval
+//    index is s >> 52 and the fraction, OR-ed under the exponent of 1.0, gives 1 + frac directly as a
+//    double: tau = (1 + frac) - 1.5 is the offset from the interval midpoint -- 1 DADD instead of the
+//    4 of a floating-point round-and-subtract, and the window below is found with the same integers.
+//  * one fused pass per pair over the window of logx intervals its energies touch: lane l contracts
+//    the mu stencil at NPL consecutive nodes (4 loads + 4 FMA each, slice rows in shared memory),
+//    takes the three neighbouring node values from lanes l-1 / l+1 by shuffle, and writes the
+//    monomial coefficients k0..k3 (in tau) of its NPL intervals -- cubic Lagrange on the 4 surrounding
+//    nodes; linear (strategy d) or the inward-shifted stencil (strategy a) in the first / last
+//    interval of the axis -- pre-scaled by log2(10), with log2(F_p T^3) added to k0.  NPL is odd so that
+//    the lanes' 8- and 16-byte accesses at stride NPL fall in distinct banks.
+//  * per triple: 2 x LDS.128 (k0..k3), Horner (3 DFMA), exp2_p10 (3 DADD + 10 DFMA), accumulate (1 DADD).
+// The division by E_e of Eq 47 is the same for every term of a bin: applied once in the epilogue.
+// ------------------------------------------------------------------------------------------------
+constexpr double kTwo52 = 4503599627370496.0;
+
+// (a & 0x000FFFFF) | 0x3FF00000 in one LOP3: the high word of 1 + frac
+__device__ __forceinline__ int one_plus_frac_hi(int shi)
+{
+    int r;
+    asm("lop3.b32 %0, %1, 0x000FFFFF, 0x3FF00000, 0xEA;" : "=r"(r) : "r"(shi));
+    return r;
+}
+
+// node value of the pair at slice column `col` of the stencil's first mu row: log2(10) * sum_mu w_mu S[mu][col] + log2(F_p T^3)
+// (the Lagrange weights of every x rule sum to 1, so adding the constant to the nodes adds it to k0 only)
+__device__ __forceinline__ double node_value(const double* __restrict__ sp0, int nx, double v0, double v1, double v2,
+                                             double v3, double qb)
+{
+    return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], fma(v0, sp0[0], qb))));
+}
+
+// monomial coefficients (in tau, the offset from the interval midpoint in units of h) of the cubic through
+// the node values c0..c3 at tau = -3/2, -1/2, 1/2, 3/2
+__device__ __forceinline__ void cubic_coeffs(double c0, double c1, double c2, double c3, double& k0, double& k1,
+                                             double& k2, double& k3)
+{
+    const double s03 = c0 + c3, s12 = c1 + c2, d30 = c3 - c0, d21 = c2 - c1;
+    k0 = fma(s03, -0.0625, s12 * 0.5625);
+    k1 = fma(d30, -1.0 / 24.0, d21 * 1.125);
+    k2 = (s03 - s12) * 0.25;
+    k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
+}
+
+template <int EPL, int NPL, int NT>
+__global__ void __launch_bounds__(NT, 1) k_cells_tab(CellArgs A)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int chunk = blockIdx.x, pg = blockIdx.y;
+    const int b = blockIdx.z / A.n_etile, et = blockIdx.z % A.n_etile;
+    const int k = pg * A.nw + w;
+    const bool kvalid = k < A.n_phase;
+    const int e0 = et * 32 * EPL;
+    const int n1 = A.n_fp + 1;
+    const int nx = A.nx;
+    const int plane = A.nmu * nx;
+    // shared layout (doubles): per warp { KA [KW] (k0,k1), KB [KW] (k2,k3), R0 [32] (q,qb), R1 [32] (v0,v1), R2 [32] (v2,v3)
+    // as double2, RI [32] int } | S [nmu][nx] | T [4][n1] | MUAX [nmu].  Struct-of-arrays so that lanes touch consecutive
+    // 16-byte words (no bank conflicts); KA / KB are indexed by node offset inside the pair's window.
+    constexpr int KW = 32 * NPL;
+    constexpr int WARP_DBL = 4 * KW + 3 * 64 + 16;
+    double* wbase = sm + (size_t)w * WARP_DBL;
+    double2* KA = reinterpret_cast<double2*>(wbase);
+    double2* R0 = KA + 2 * KW;
+    double2* R1 = R0 + 32;
+    double2* R2 = R1 + 32;
+    int* RI = reinterpret_cast<int*>(R2 + 32);
+    double* S = sm + (size_t)A.nw * WARP_DBL;
+    double* T = S + plane;
+    double* MUAX = T + 4 * n1;
+
+    long long uef[EPL];
+    double acc[EPL];
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) {
+        const int e = e0 + lane + 32 * i;
+        uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
+        acc[i] = 0.0;
+    }
+    const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
+    const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
+    const long long s_top = ((long long)(nx - 1) << 52) - 1;                     // largest in-table coordinate
+    for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
+
+    const StarD& st = A.stars[b];
+    const double phi_off = st.phi_off;
+    const double phi_out = (double)k / A.n_phase;                               // reading R3
+    unsigned npairs = 0;
+
+    for (int ri = 0; ri < A.rows_per_chunk; ++ri) {
+        const int rl = chunk + ri * A.nchunk;                                   // strided chunks balance row sizes
+        if (rl >= A.RT) break;
+        const int rid = b * A.RT + rl;
+        const RowD& row = A.rows[rid];
+        const int nact = row.n_active;
+        if (nact == 0 || !row.visible) continue;
+        const SpotD& sp = A.spots[rid / A.n_theta];
+        __syncthreads();
+        {   // stage slice + template (16-byte loads)
+            if ((plane & 1) == 0) {
+                const double2* src = reinterpret_cast<const double2*>(A.slices + (size_t)rid * plane);
+                double2* dst = reinterpret_cast<double2*>(S);
+                for (int i = threadIdx.x; i < plane / 2; i += blockDim.x) dst[i] = src[i];
+            } else {
+                const double* src = A.slices + (size_t)rid * plane;
+                for (int i = threadIdx.x; i < plane; i += blockDim.x) S[i] = src[i];
+            }
+            const double* ts = A.tmpl + (size_t)rid * 4 * n1;
+            for (int i = threadIdx.x; i < 4 * n1; i += blockDim.x) T[i] = ts[i];
+        }
+        __syncthreads();
+        if (!kvalid) continue;
+        const double* F = T;
+        const double* Z = T + n1;
+        const double* PO = T + 2 * n1;
+        const double* MU = T + 3 * n1;
+        const int* cl = A.cells + (size_t)rid * A.n_phi;
+        const double po0 = PO[0];
+        for (int base = 0; base < nact; base += 32) {
+            // ---- step A: lane <-> cell; Eq 45-46 and the per-pair record, compacted over the pairs with F_p != 0 ----
+            const int idx = base + lane;
+            double Fp = 0.0, pb = 0.0;                // pb = log2(F_p T^3)
+            long long pq = 0;                         // u_pair in units of 2^-52 intervals
+            double ww[4] = {0.0, 0.0, 0.0, 0.0};
+            int info = 0;                             // slice offset of the mu stencil's first row | jlo << 16 | jhi << 24
+            if (idx < nact) {
+                const int m = cl[idx];
+                const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
+                const double phi_m = sp.phi_c + dphi_m;
+                const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
+                const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
+                int lo = 0, hi = A.n_fp;
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (PO[mid] <= phi_p) lo = mid; else hi = mid;
+                }
+                const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
+                Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                           // Eq 46, linear (reading R11)
+                const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
+                const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+                if (Fp != 0.0) {
+                    const double up = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h;   // (x - x0)/h less the energy part
+                    pq = __double2ll_rn(up * kTwo52);
+                    pb = log2(Fp) + sp.log2T3;
+                    int mb;
+                    axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= kLog2_10;
+                    // window of logx intervals touched by this pair's energies (coordinates clamped to the table, reading R13b)
+                    const long long sa = pq + uef_first, sb2 = pq + uef_last;
+                    const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
+                    const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
+                    const int clamped = (sa < 0) || (sb2 > s_top);
+                    info = (mb * nx) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
+                }
+            }
+            const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);
+            const int cnt = __popc(valid);
+            npairs += cnt;
+            __syncwarp();
+            if (Fp != 0.0) {
+                const int slot = __popc(valid & ((1u << lane) - 1u));
+                R0[slot] = make_double2(__longlong_as_double(pq), pb);
+                R1[slot] = make_double2(ww[0], ww[1]);
+                R2[slot] = make_double2(ww[2], ww[3]);
+                RI[slot] = info;
+            }
+            __syncwarp();
+            // ---- step B: walk the valid pairs ----
+            for (int pj = 0; pj < cnt; ++pj) {
+                const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj];
+                const int inf = RI[pj];
+                const long long q = __double_as_longlong(r0.x);
+                const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
+                const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
+                const double* srow = S + (inf & 0x7FFF);
+                // ---- fused pass: node values -> interval coefficients.  Lane l holds nodes n0 .. n0+NPL-1, n0 = jlo-1 + NPL l;
+                // interval c (nodes c, c+1) has window offset c - (jlo-1).  Out-of-table nodes read neighbouring shared memory:
+                // they only feed window slots that no energy reads.
+                const int n0 = jlo - 1 + NPL * lane;
+                const double* sp0 = srow + n0;
+                double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
+#pragma unroll
+                for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node_value(sp0 + jn, nx, v0, v1, v2, v3, qb);
+                f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
+                if (NPL == 1) {
+                    f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
+                    f[3] = __shfl_down_sync(0xffffffffu, f[1], 2);
+                } else {
+                    f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
+                    f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
+                }
+                double2 ka[NPL], kb[NPL];
+#pragma unroll
+                for (int jn = 0; jn < NPL; ++jn) cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
+                if (jlo == 0 || jhi == nx - 2) {      // the window holds the first / last interval of the axis (warp-uniform)
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn) {
+                        const int c = n0 + jn;
+                        if (c != 0 && c != nx - 2) continue;
+                        if (A.x_linedge) {                                      // strategy d: linear
+                            ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
+                            kb[jn] = make_double2(0.0, 0.0);
+                        } else {                                                // strategy a: stencil shifted inward
+                            const int s = (c == 0) ? 0 : nx - 4;
+                            double g[4];
+#pragma unroll
+                            for (int m = 0; m < 4; ++m) g[m] = node_value(srow + s + m, nx, v0, v1, v2, v3, qb);
+                            double k0, k1, k2, k3;
+                            cubic_coeffs(g[0], g[1], g[2], g[3], k0, k1, k2, k3);
+                            const double d = (double)(c - 1 - s);               // Taylor shift to this interval's midpoint
+                            ka[jn] = make_double2(fma(d, fma(d, fma(d, k3, k2), k1), k0), fma(d, fma(3.0 * d, k3, 2.0 * k2), k1));
+                            kb[jn] = make_double2(fma(3.0 * d, k3, k2), k3);
+                        }
+                    }
+                }
+                __syncwarp();                                                   // the previous pair's readers are done
+#pragma unroll
+                for (int jn = 0; jn < NPL; ++jn) {
+                    KA[NPL * lane + jn] = ka[jn];
+                    KA[NPL * lane + jn + KW] = kb[jn];
+                }
+                __syncwarp();
+                const double2* KAq = KA + (1 - jlo);
+                // ---- energies ----
+                if (!(inf & 0x8000)) {
+#pragma unroll
+                    for (int i = 0; i < EPL; ++i) {
+                        const long long s = q + uef[i];
+                        const int shi = (int)(s >> 32);
+                        const double2* kp = KAq + (shi >> 20);                  // interval index = s >> 52
+                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                        const double2 c01 = kp[0], c23 = kp[KW];
+                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+                        const double r = y + kMagic;
+                        const int n = __double2loint(r);
+                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
+                        if (n >= -1000) acc[i] += val;
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < EPL; ++i) {
+                        long long s = q + uef[i];
+                        s = s < 0 ? 0 : (s > s_top ? s_top : s);                 // clamp to the table (reading R13b)
+                        const int shi = (int)(s >> 32);
+                        const double2* kp = KAq + (shi >> 20);
+                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                        const double2 c01 = kp[0], c23 = kp[KW];
+                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+                        const double r = y + kMagic;
+                        const int n = __double2loint(r);
+                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
+                        if (n >= -1000) acc[i] += val;
+                    }
+                }
+            }
+        }
+    }
+    if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
+    if (kvalid) {
+        double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) {
+            const int e = e0 + lane + 32 * i;
+            if (e < A.nE) out[e] = acc[i] / A.en[e];                            // the 1/E_e of Eq 47
         }
     }
 }
