@@ -122,6 +122,7 @@ struct ppm_ctx {
     StarD* d_stars = nullptr; SpotD* d_spots = nullptr; RowD* d_rows = nullptr; int* d_cells = nullptr;
     double *d_lookup = nullptr, *d_tmpl = nullptr, *d_slices = nullptr, *d_partial = nullptr;
     double* d_lgam = nullptr;
+    double* d_llpart = nullptr; int* d_llbad = nullptr; int llpart_cap = 0;   // ln L slice sums [cap][kLLSplit]
     // host-variant staging
     double *d_params_stage = nullptr, *d_flux_stage = nullptr, *d_ll_stage = nullptr, *d_counts_stage = nullptr;
     int* d_status_stage = nullptr;
@@ -167,6 +168,8 @@ extern "C" int ppm_destroy(ppm_ctx* c)
                     c->d_ll_stage, c->d_counts_stage, c->d_status_stage};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (c->d_pairs) cudaFree(c->d_pairs);
+    if (c->d_llpart) cudaFree(c->d_llpart);
+    if (c->d_llbad) cudaFree(c->d_llbad);
     for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     delete c;
     return PPM_OK;
@@ -216,18 +219,13 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     c->n_fp = cfg->n_fp > 0 ? cfg->n_fp : std::max(192, 2 * cfg->n_phase);           // reading R2
     c->h_en.assign(energies, energies + cfg->n_energy);
     // launch geometry of the cell kernel
-    // experiment knobs (to be frozen): PPM_CELLS_NW warps per block (16 or 32), PPM_CELLS_EPL energies per lane
-    const char* env_nw = getenv("PPM_CELLS_NW");
-    const char* env_epl = getenv("PPM_CELLS_EPL");
-    const int nw_max = (env_nw && cfg->emission != PPM_EMISSION_BLACKBODY) ? atoi(env_nw) : 16;
-    c->nw = std::min(nw_max, cfg->n_phase);
+    // 16 warps x 128 registers fill the register file; 32 warps x 64 registers measured slower (profiles/r1c_variants.md)
+    c->nw = std::min(16, cfg->n_phase);
     c->npg = (cfg->n_phase + c->nw - 1) / c->nw;
     const int need = (cfg->n_energy + 31) / 32;
     const int epls[] = {1, 2, 4, 5, 8, 10};
     c->epl = 10;
     for (int v : epls) if (v >= need) { c->epl = v; break; }
-    if (env_epl && cfg->emission != PPM_EMISSION_BLACKBODY) c->epl = atoi(env_epl);
-    if (c->nw > 16 && c->epl > 5) c->epl = 5;
     c->n_etile = (cfg->n_energy + 32 * c->epl - 1) / (32 * c->epl);
     const double per_row = (double)cfg->n_phase * cfg->n_energy * 8.0;
     c->rows_per_chunk = 1;
@@ -306,7 +304,6 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     }
     c->npl = 1;
     while (32 * c->npl - 3 < c->wmax) c->npl += 2;                 // odd: conflict-free strided shared-memory accesses
-    if (getenv("PPM_CELLS_NPL2") && 61 >= c->wmax) c->npl = 2;
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;
@@ -359,46 +356,37 @@ static int launch_cells(ppm_ctx* c, K kernel, const CellArgs& a, dim3 grid, int 
     return PPM_OK;
 }
 
-template <int EPL, int NT>
+template <int EPL>
 static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
     switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_tab<EPL, 1, NT>, a, grid, threads, smem);
-    case 2:  return launch_cells(c, k_cells_tab<EPL, 2, NT>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_tab<EPL, 3, NT>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_tab<EPL, 5, NT>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_tab<EPL, 7, NT>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_tab<EPL, 9, NT>, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_tab<EPL, 3>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_tab<EPL, 5>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_tab<EPL, 7>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_tab<EPL, 9>, a, grid, threads, smem);
     }
 }
 
 static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
-    if (table && threads > 512) {
-        switch (c->epl) {
-        case 1:  return dispatch_cells_tab<1, 1024>(c, a, grid, threads, smem);
-        case 2:  return dispatch_cells_tab<2, 1024>(c, a, grid, threads, smem);
-        case 4:  return dispatch_cells_tab<4, 1024>(c, a, grid, threads, smem);
-        default: return dispatch_cells_tab<5, 1024>(c, a, grid, threads, smem);
-        }
-    }
     if (table) {
         switch (c->epl) {
-        case 1:  return dispatch_cells_tab<1, 512>(c, a, grid, threads, smem);
-        case 2:  return dispatch_cells_tab<2, 512>(c, a, grid, threads, smem);
-        case 4:  return dispatch_cells_tab<4, 512>(c, a, grid, threads, smem);
-        case 5:  return dispatch_cells_tab<5, 512>(c, a, grid, threads, smem);
-        case 8:  return dispatch_cells_tab<8, 512>(c, a, grid, threads, smem);
-        default: return dispatch_cells_tab<10, 512>(c, a, grid, threads, smem);
+        case 1:  return dispatch_cells_tab<1>(c, a, grid, threads, smem);
+        case 2:  return dispatch_cells_tab<2>(c, a, grid, threads, smem);
+        case 4:  return dispatch_cells_tab<4>(c, a, grid, threads, smem);
+        case 5:  return dispatch_cells_tab<5>(c, a, grid, threads, smem);
+        case 8:  return dispatch_cells_tab<8>(c, a, grid, threads, smem);
+        default: return dispatch_cells_tab<10>(c, a, grid, threads, smem);
         }
     }
     switch (c->epl) {
-    case 1:  return launch_cells(c, k_cells<1, 0>, a, grid, threads, smem);
-    case 2:  return launch_cells(c, k_cells<2, 0>, a, grid, threads, smem);
-    case 4:  return launch_cells(c, k_cells<4, 0>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells<5, 0>, a, grid, threads, smem);
-    case 8:  return launch_cells(c, k_cells<8, 0>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells<10, 0>, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells_bb<1>, a, grid, threads, smem);
+    case 2:  return launch_cells(c, k_cells_bb<2>, a, grid, threads, smem);
+    case 4:  return launch_cells(c, k_cells_bb<4>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_bb<5>, a, grid, threads, smem);
+    case 8:  return launch_cells(c, k_cells_bb<8>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_bb<10>, a, grid, threads, smem);
     }
 }
 
@@ -420,7 +408,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     k_rows<<<rows, 128, 0, c->stream>>>(G);
     prof_end(c);
     prof_begin(c, KID_LOOKUP);
-    k_lookup<<<rows, kNCheb, 0, c->stream>>>(G);
+    k_lookup<<<rows, kNCheb * kNGL, 0, c->stream>>>(G);
     prof_end(c);
     const size_t tsm = sizeof(double) * (2 * kNCheb + 4 * (size_t)(c->n_fp + 1));
     if (tsm > 48 * 1024) CK(cudaFuncSetAttribute(k_template, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
@@ -534,10 +522,22 @@ extern "C" int ppm_loglike(ppm_ctx* c, const double* counts_dev, int B, const do
     if (B == 0) return PPM_OK;
     CK(cudaSetDevice(c->cfg.device));
     prof_begin(c, KID_LOGLIKE);
-    k_loglike<<<1, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
-                                        nullptr, 1, c->d_lgam);
-    k_loglike<<<B, 512, 0, c->stream>>>(counts_dev, data_dev, bkg_dev, c->cfg.n_phase, c->n_channel, exposure_s,
-                                        c->d_lgam, 0, loglike_dev);
+    for (int b0 = 0; b0 < B; b0 += 32768) {
+        const int nb = std::min(32768, B - b0);
+        if (!c->d_llpart || c->llpart_cap < nb + 1) {
+            if (c->d_llpart) cudaFree(c->d_llpart);
+            if (c->d_llbad) cudaFree(c->d_llbad);
+            c->d_llpart = nullptr; c->d_llbad = nullptr;
+            int rc;
+            if ((rc = dev_alloc(&c->d_llpart, (size_t)(nb + 1) * kLLSplit)) || (rc = dev_alloc(&c->d_llbad, (size_t)(nb + 1) * kLLSplit)))
+                return rc;
+            c->llpart_cap = nb + 1;
+        }
+        dim3 grid(kLLSplit, nb + 1);
+        k_loglike_part<<<grid, 256, 0, c->stream>>>(counts_dev + (size_t)b0 * c->cfg.n_phase * c->n_channel, data_dev, bkg_dev,
+                                                    c->cfg.n_phase, c->n_channel, exposure_s, nb, c->d_llpart, c->d_llbad);
+        k_loglike_final<<<(nb + 127) / 128, 128, 0, c->stream>>>(c->d_llpart, c->d_llbad, nb, loglike_dev + b0);
+    }
     prof_end(c);
     c->launches += 2;
     CK(cudaGetLastError());

@@ -56,9 +56,9 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
     A.slices[(size_t)rid * plane + i] = v;
 }
 
-// 2^y for the table path: y = n + f, n = round(y) through the 1.5*2^52 constant, |f| <= 1/2;
+// 2^y for the table path: y = n + f, n = round(y) through the 1.5*2^52 constant (done by the caller), |f| <= 1/2;
 // 2^f by a degree-10 polynomial (Chebyshev-node fit on [-1/2, 1/2]; max relative error 4.3e-16 in double
-// arithmetic), 2^n by an integer add into the exponent field.  y < -1000 -> 0.
+// arithmetic), 2^n by an integer add into the exponent field.  The caller drops terms with n < -1000.
 __device__ __forceinline__ double exp2_frac_scaled(double f, int n)      // 2^f * 2^n, |f| <= 1/2, no range check
 {
     double p = 7.072585949269223e-09;
@@ -75,44 +75,17 @@ __device__ __forceinline__ double exp2_frac_scaled(double f, int n)      // 2^f 
     return __hiloint2double(__double2hiint(p) + n * 1048576, __double2loint(p));
 }
 
-__device__ __forceinline__ double exp2_p10(double y)
-{
-    const double r = y + kMagic;
-    const int n = __double2loint(r);
-    const double f = y - (r - kMagic);
-    double p = 7.072585949269223e-09;
-    p = fma(p, f, 1.0208690299958306e-07);
-    p = fma(p, f, 1.321544258792169e-06);
-    p = fma(p, f, 1.5252657260200837e-05);
-    p = fma(p, f, 0.0001540353044173605);
-    p = fma(p, f, 0.0013333558230164974);
-    p = fma(p, f, 0.009618129107606888);
-    p = fma(p, f, 0.05550410866444772);
-    p = fma(p, f, 0.24022650695910097);
-    p = fma(p, f, 0.69314718055995);
-    p = fma(p, f, 1.0);
-    const int hi = __double2hiint(p) + n * 1048576;
-    return (n < -1000) ? 0.0 : __hiloint2double(hi, __double2loint(p));
-}
 
 // ------------------------------------------------------------------------------------------------
-// K5: shift-and-add.  Block = (row chunk, group of `nw` consecutive output phases, vector x energy
-// tile); warp w owns output phase k and the 32*EPL energies of the tile (lane owns energies
-// e0+lane+32 i): the (k, e) accumulators live in registers for the whole chunk -- output-stationary,
-// no atomics.  Per row the (mu x logx) slice and the ring template sit in shared memory.  Lanes first
-// prepare 32 (cell, k) pairs in parallel (Eq 45-46, mu stencil, the window of logx intervals the pair's
-// energies fall in), then the warp walks the pairs with F_p != 0.  Per pair (work shared by all its
-// energies): contract the mu stencil into node values over the window, then turn every interval of
-// the window into the monomial coefficients k0..k3 of its interpolating polynomial in
-// tau = (x - x_mid)/h (cubic Lagrange on the 4 surrounding nodes; linear / shifted stencil in the edge
-// intervals per strategy), pre-scaled by log2(10) and with log2(F_p T^3) added to k0.  Per triple:
-// interval index + tau (4 DADD), Horner (3 DFMA), exp2_p10 (3 DADD + 10 DFMA), accumulate (1 DADD).
-// The division by E_e of Eq 47 is the same for every term of a bin and is applied once in the epilogue.
-// MODE 0: closed-form isotropic blackbody (Eq C.5); MODE 1: table.
+// K5: shift-and-add (Eq 45-47).  Block = (row chunk, group of `nw` consecutive output
+// phases, vector x energy tile); warp w owns output phase k and the 32*EPL energies of the tile (lane
+// owns energies e0+lane+32 i): the (k, e) accumulators live in registers for the whole chunk --
+// output-stationary, no atomics.  Per row the ring template sits in shared memory.  Lanes first prepare
+// 32 (cell, k) pairs in parallel (Eq 45-46), then the warp walks the pairs with F_p != 0.
+// k_cells_bb: closed-form isotropic blackbody (Eq C.5).  k_cells_tab (below): table.
 // ------------------------------------------------------------------------------------------------
-
-template <int EPL, int MODE>
-__global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
+template <int EPL>
+__global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -122,38 +95,16 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
     const bool kvalid = k < A.n_phase;
     const int e0 = et * 32 * EPL;
     const int n1 = A.n_fp + 1;
-    const int nx = A.nx;
-    const int plane = (MODE == 1) ? A.nmu * nx : 0;
-    // shared layout: per warp KA [wmax] (k0, k1), KB [wmax] (k2, k3) as double2 (16-byte aligned; two arrays so that
-    // lanes writing / reading consecutive intervals touch consecutive 16-byte words: no bank conflicts)
-    // | S [nmu][nx] | T [4][n1] | MUAX [nmu] | CV per warp [nx]
-    const int kc_len = (MODE == 1) ? 4 * A.wmax : 0;
-    double* KCall = sm;
-    double* S = KCall + (size_t)A.nw * kc_len;
-    double* T = S + plane;
-    double* MUAX = T + 4 * n1;
-    double* CV = MUAX + ((MODE == 1) ? A.nmu : 0) + (size_t)w * nx;
-    double2* KA = reinterpret_cast<double2*>(KCall + (size_t)w * kc_len);
-    double2* KB = KA + A.wmax;
+    double* T = sm;                                  // F, z, phi_o, mu: [4][n1]
 
-    double ue[EPL], c2[(MODE == 0) ? EPL : 1], acc[EPL];
+    double en[EPL], ok[EPL], acc[EPL];
 #pragma unroll
     for (int i = 0; i < EPL; ++i) {
         const int e = e0 + lane + 32 * i;
-        const bool ok = e < A.nE;
-        if (MODE == 1) {
-            ue[i] = A.ue[ok ? e : A.nE - 1];
-        } else {
-            ue[i] = ok ? A.en[e] : 1.0;              // E_e
-            c2[i] = ok ? 1.0 : 0.0;
-        }
+        en[i] = (e < A.nE) ? A.en[e] : 1.0;
+        ok[i] = (e < A.nE) ? 1.0 : 0.0;
         acc[i] = 0.0;
     }
-    const int e_last = imin_(e0 + 32 * EPL, A.nE) - 1;
-    const double ue_first = (MODE == 1) ? A.ue[imin_(e0, A.nE - 1)] : 0.0;
-    const double ue_last = (MODE == 1) ? A.ue[e_last] : 0.0;
-    if (MODE == 1) for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
-
     const StarD& st = A.stars[b];
     const double phi_off = st.phi_off;
     const double phi_out = (double)k / A.n_phase;                               // reading R3
@@ -168,32 +119,18 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
         if (nact == 0 || !row.visible) continue;
         const SpotD& sp = A.spots[rid / A.n_theta];
         __syncthreads();
-        {   // stage slice + template (16-byte loads)
-            if ((plane & 1) == 0 && ((A.nw * kc_len) & 1) == 0) {
-                const double2* src = reinterpret_cast<const double2*>(A.slices + (size_t)rid * plane);
-                double2* dst = reinterpret_cast<double2*>(S);
-                for (int i = threadIdx.x; i < plane / 2; i += blockDim.x) dst[i] = src[i];
-            } else {
-                const double* src = A.slices + (size_t)rid * plane;
-                for (int i = threadIdx.x; i < plane; i += blockDim.x) S[i] = src[i];
-            }
-            const double* ts = A.tmpl + (size_t)rid * 4 * n1;
-            for (int i = threadIdx.x; i < 4 * n1; i += blockDim.x) T[i] = ts[i];
-        }
+        const double* ts = A.tmpl + (size_t)rid * 4 * n1;
+        for (int i = threadIdx.x; i < 4 * n1; i += blockDim.x) T[i] = ts[i];
         __syncthreads();
         if (!kvalid) continue;
         const double* F = T;
         const double* Z = T + n1;
         const double* PO = T + 2 * n1;
-        const double* MU = T + 3 * n1;
         const int* cl = A.cells + (size_t)rid * A.n_phi;
         const double po0 = PO[0];
         for (int base = 0; base < nact; base += 32) {
-            // ---- step A: lane <-> cell; Eq 45-46 and the per-pair constants ----
             const int idx = base + lane;
-            double Fp = 0.0, pa = 0.0, pb = 0.0;      // MODE 1: pa = uz, pb = log2(F_p T^3);  MODE 0: pa = z_p / kT, pb = F_p z_p^3 K
-            double w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0;
-            int info = 0;                             // MODE 1: mu stencil base | jlo << 7 | jhi << 15 | fast << 23
+            double Fp = 0.0, pa = 0.0, pb = 0.0;      // pa = z_p / kT, pb = F_p z_p^3 2/(h^3 c^2)
             if (idx < nact) {
                 const int m = cl[idx];
                 const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
@@ -208,112 +145,22 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
                 const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
                 Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                           // Eq 46, linear (reading R11)
                 const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
-                const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
                 if (Fp != 0.0) {
-                    if (MODE == 1) {
-                        pa = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h - 0.5;   // (x - x0)/h - 0.5, less the energy part
-                        pb = log2(Fp) + sp.log2T3;
-                        double ww[4];
-                        int mb;
-                        axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
-                        w0 = ww[0] * kLog2_10; w1 = ww[1] * kLog2_10; w2 = ww[2] * kLog2_10; w3 = ww[3] * kLog2_10;
-                        // window of logx intervals touched by this pair's energies, found with the very arithmetic
-                        // the energy loop uses (monotone in e, so first / last energy bound every index)
-                        const double hi_c = (double)nx - 1.5;
-                        const double ua = pa + ue_first, ub = pa + ue_last;
-                        const int fast = (ua >= -0.5) && (ub < hi_c);
-                        const int jlo = imin_(__double2loint(fmin(fmax(ua, -0.5), hi_c) + kMagic), nx - 2);
-                        const int jhi = imin_(__double2loint(fmin(fmax(ub, -0.5), hi_c) + kMagic), nx - 2);
-                        info = mb | (jlo << 7) | (jhi << 15) | (fast << 23);
-                    } else {
-                        pa = zp / sp.kT;
-                        pb = Fp * (2.0 / (kH_keV_s * kH_keV_s * kH_keV_s * kC_cm_s * kC_cm_s)) * zp * zp * zp;
-                    }
+                    pa = zp / sp.kT;
+                    pb = Fp * (2.0 / (kH_keV_s * kH_keV_s * kH_keV_s * kC_cm_s * kC_cm_s)) * zp * zp * zp;
                 }
             }
             unsigned todo = __ballot_sync(0xffffffffu, Fp != 0.0);
             npairs += __popc(todo);
-            // ---- step B: walk the valid pairs ----
             while (todo) {
                 const int j = __ffs(todo) - 1;
                 todo &= todo - 1;
                 const double qa = __shfl_sync(0xffffffffu, pa, j);
                 const double qb = __shfl_sync(0xffffffffu, pb, j);
-                if constexpr (MODE == 0) {
 #pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        const double E = ue[i];
-                        acc[i] += c2[i] * (qb * E * E / expm1(qa * E));         // F_p I(z_p E)/E, Eq 47 with Eq C.5
-                    }
-                    continue;
-                }
-                const double v0 = __shfl_sync(0xffffffffu, w0, j);
-                const double v1 = __shfl_sync(0xffffffffu, w1, j);
-                const double v2 = __shfl_sync(0xffffffffu, w2, j);
-                const double v3 = __shfl_sync(0xffffffffu, w3, j);
-                const int inf = __shfl_sync(0xffffffffu, info, j);
-                const int sb = inf & 127, jlo = (inf >> 7) & 255, jhi = (inf >> 15) & 255;
-                const bool fast = (inf >> 23) & 1;
-                // node values log2(10) * sum_mu w_mu S[mu][c] on the nodes the window's stencils touch
-                const int nlo = imin_(imax_(jlo - 1, 0), nx - 4);
-                const int nhi = imin_(imax_(jhi + 2, nlo + 3), nx - 1);
-                __syncwarp();
-                {
-                    const double* sp0 = S + sb * nx + nlo + lane;
-                    double* cv = CV + nlo + lane;
-                    for (int c = nlo + lane; c <= nhi; c += 32, sp0 += 32, cv += 32)
-                        *cv = fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
-                }
-                __syncwarp();
-                // per interval c in [jlo, jhi]: monomial coefficients in tau (offset from the interval midpoint, in units of h)
-                for (int c = jlo + lane; c <= jhi; c += 32) {
-                    const int s = imin_(imax_(c - 1, 0), nx - 4);
-                    const double* cvs = CV + s;
-                    const double c0 = cvs[0], c1 = cvs[1], c2v = cvs[2], c3 = cvs[3];
-                    const double s03 = c0 + c3, s12 = c1 + c2v, d30 = c3 - c0, d21 = c2v - c1;
-                    double k0 = fma(s03, -0.0625, s12 * 0.5625);
-                    double k1 = fma(d30, -1.0 / 24.0, d21 * 1.125);
-                    double k2 = (s03 - s12) * 0.25;
-                    double k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
-                    if (s != c - 1) {                                           // first / last interval of the axis
-                        if (A.x_linedge) {                                      // strategy d: linear
-                            const double a = CV[c], bb = CV[c + 1];
-                            k0 = 0.5 * (a + bb); k1 = bb - a; k2 = 0.0; k3 = 0.0;
-                        } else {                                                // strategy a: shifted stencil, Taylor shift by d
-                            const double d = (double)(c - 1 - s);
-                            k0 = fma(d, fma(d, fma(d, k3, k2), k1), k0);
-                            k1 = fma(d, fma(3.0 * d, k3, 2.0 * k2), k1);
-                            k2 = fma(3.0 * d, k3, k2);
-                        }
-                    }
-                    KA[c - jlo] = make_double2(k0 + qb, k1);
-                    KB[c - jlo] = make_double2(k2, k3);
-                }
-                __syncwarp();
-                const double2* KAj = KA - jlo;
-                const double2* KBj = KB - jlo;
-                if (fast) {
-#pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        const double uu = qa + ue[i];                           // (x - x0)/h - 0.5
-                        const double r = uu + kMagic;
-                        const int ii = __double2loint(r);                       // interval index, x in [x_ii, x_ii+1]
-                        const double tau = uu - (r - kMagic);                   // offset from the interval midpoint
-                        const double2 ka = KAj[ii], kb = KBj[ii];
-                        acc[i] += exp2_p10(fma(fma(fma(kb.y, tau, kb.x), tau, ka.y), tau, ka.x));
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        // clamp (x - x0)/h to [0, nx-1] (reading R13b); a tie at the upper end may round to interval nx-1
-                        const double uu = fmin(fmax(qa + ue[i], -0.5), (double)nx - 1.5);
-                        const double r = uu + kMagic;
-                        int ii = __double2loint(r);
-                        double tau = uu - (r - kMagic);
-                        if (ii > nx - 2) { ii = nx - 2; tau += 1.0; }
-                        const double2 ka = KAj[ii], kb = KBj[ii];
-                        acc[i] += exp2_p10(fma(fma(fma(kb.y, tau, kb.x), tau, ka.y), tau, ka.x));
-                    }
+                for (int i = 0; i < EPL; ++i) {
+                    const double E = en[i];
+                    acc[i] += ok[i] * (qb * E * E / expm1(qa * E));             // F_p I(z_p E)/E, Eq 47 with Eq C.5
                 }
             }
         }
@@ -324,7 +171,7 @@ __global__ void __launch_bounds__(512, 1) k_cells(CellArgs A)
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
             const int e = e0 + lane + 32 * i;
-            if (e < A.nE) out[e] = (MODE == 1) ? acc[i] / A.en[e] : acc[i];    // the 1/E_e of Eq 47
+            if (e < A.nE) out[e] = acc[i];
         }
     }
 }
@@ -378,8 +225,8 @@ __device__ __forceinline__ void cubic_coeffs(double c0, double c1, double c2, do
     k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
 }
 
-template <int EPL, int NPL, int NT>
-__global__ void __launch_bounds__(NT, 1) k_cells_tab(CellArgs A)
+template <int EPL, int NPL>
+__global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;

@@ -20,38 +20,37 @@ __constant__ double c_glw[kNGL];   // weights
 // panel the nearest complex singularity is >= one panel width away, which makes the rule converge to
 // round-off (S2).
 // ------------------------------------------------------------------------------------------------
-__device__ inline void geo_panel(double a, double b, double k, double sa2, double ca2, double& I1, double& I2)
-{
-    const double hm = 0.5 * (b - a), c = 0.5 * (a + b);
-    double s1 = 0.0, s2 = 0.0;
-#pragma unroll 4
-    for (int i = 0; i < kNGL; ++i) {
-        const double x = fma(hm, c_glx[i], c);
-        const double x2 = x * x, om = 1.0 - x2;
-        const double q = (2.0 - x2 - k * om * om) * sa2;
-        const double D = fma(x2, q, ca2);
-        const double sD = sqrt(D);
-        const double t = c_glw[i] * x / sD;
-        s1 += t;
-        s2 += t / (1.0 + sD);
-    }
-    I1 = fma(hm, s1, I1);
-    I2 = fma(hm, s2, I2);
-}
-
-__device__ inline void geo_integrals(double u, double sa, double cabs, double& I1, double& I2)
+// Cooperative form: a group of kNGL = 16 adjacent lanes integrates one (u, alpha); lane g of the group owns
+// Gauss-Legendre point g of every panel, the group sums by xor-shuffles after the panel loop (all 32 lanes of
+// the warp must call these functions together; the two groups of a warp may run different panel counts).
+__device__ inline void geo_integrals(double u, double sa, double cabs, int g, double& I1, double& I2)
 {
     const double k = u / (1.0 - u), sa2 = sa * sa, ca2 = cabs * cabs;
     const double q0 = (2.0 - k) * sa2;
     const double layer = (q0 > 0.0) ? cabs / sqrt(q0) : 1.0;
-    I1 = 0.0; I2 = 0.0;
+    const double gx = c_glx[g], gw = c_glw[g];
+    double s1 = 0.0, s2 = 0.0;
     double hi = 1.0;
-    for (int p = 0; p < kMaxPanels && hi > layer; ++p) {
-        const double lo = 0.5 * hi;
-        geo_panel(lo, hi, k, sa2, ca2, I1, I2);
+    bool last = false;
+    for (int p = 0; p <= kMaxPanels && !last; ++p) {
+        last = (p == kMaxPanels) || !(hi > layer);
+        const double lo = last ? 0.0 : 0.5 * hi;                 // dyadic panels [hi/2, hi], then [0, hi]
+        const double hm = 0.5 * (hi - lo), c = 0.5 * (lo + hi);
+        const double x = fma(hm, gx, c);
+        const double x2 = x * x, om = 1.0 - x2;
+        const double q = (2.0 - x2 - k * om * om) * sa2;
+        const double sD = sqrt(fma(x2, q, ca2));
+        const double t = hm * gw * x / sD;
+        s1 += t;
+        s2 += t / (1.0 + sD);
         hi = lo;
     }
-    geo_panel(0.0, hi, k, sa2, ca2, I1, I2);
+#pragma unroll
+    for (int m = kNGL / 2; m > 0; m >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, m);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, m);
+    }
+    I1 = s1; I2 = s2;
 }
 
 // psi(u, alpha) and lag(u, alpha) = (c Delta t - c delta t(R)) / R for 0 < alpha < pi.
@@ -59,21 +58,24 @@ __device__ inline void geo_integrals(double u, double sa, double cabs, double& I
 // read dimensionally (reading R6), everything divided by R:
 //   psi = 2 psi(u/rho, pi/2) - psi(u, pi - alpha)
 //   lag = 2 rho G(u/rho, pi/2) - G(u, pi - alpha) + 2 [1 - rho + u ln((1-u)/(rho-u))]
-__device__ inline void geo_psi_lag(double u, double alpha, double& psi, double& lag)
+__device__ inline void geo_psi_lag(double u, double alpha, int g, double& psi, double& lag)
 {
     double sa, ca;
     sincos(alpha, &sa, &ca);
     double I1, I2;
-    geo_integrals(u, sa, fabs(ca), I1, I2);
+    geo_integrals(u, sa, fabs(ca), g, I1, I2);
     const double psi_o = 2.0 * sa / sqrt(1.0 - u) * I1;
     const double G_o = 2.0 * sa * sa / (1.0 - u) * I2;
-    if (alpha <= 0.5 * kPi) { psi = psi_o; lag = G_o; return; }
+    const bool inward = alpha > 0.5 * kPi;
+    // the periastron integrals are needed by inward rays only; the call is warp-uniform (outgoing groups of a warp
+    // that holds an inward ray discard theirs)
     const double s3 = sqrt(3.0 * (1.0 - u));
     const double arg = fmin(3.0 * u * s3 / (2.0 * sa), 1.0);
-    const double rho = -2.0 * sa / s3 * cos((acos(arg) + 2.0 * kPi) / 3.0);      // Eq 14
+    const double rho = inward ? -2.0 * sa / s3 * cos((acos(arg) + 2.0 * kPi) / 3.0) : 1.0;      // Eq 14
     const double up = u / rho;
-    double J1, J2;
-    geo_integrals(up, 1.0, 0.0, J1, J2);
+    double J1 = 0.0, J2 = 0.0;
+    if (__any_sync(0xffffffffu, inward)) geo_integrals(up, 1.0, 0.0, g, J1, J2);
+    if (!inward) { psi = psi_o; lag = G_o; return; }
     const double psi_p = 2.0 / sqrt(1.0 - up) * J1;
     const double G_p = 2.0 / (1.0 - up) * J2;
     psi = 2.0 * psi_p - psi_o;
@@ -266,34 +268,32 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
 // Chebyshev coefficients.  u is constant along a row, so the table is 1-D in the emission angle and
 // indexed by the row (= compactness).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kNCheb) k_lookup(GeoArgs A)
+__global__ void __launch_bounds__(kNCheb * kNGL) k_lookup(GeoArgs A)
 {
-    __shared__ double fH[kNCheb], fG[kNCheb];
+    __shared__ double fH[kNCheb], fG[kNCheb], ctab[4 * kNCheb];
     const int rid = blockIdx.x;
     const RowD r = A.rows[rid];
     if (r.n_active == 0) return;
-    const int j = threadIdx.x;
+    const int j = threadIdx.x / kNGL, g = threadIdx.x % kNGL;    // Chebyshev node, Gauss-Legendre point
     const double s = cospi((2.0 * j + 1.0) / (2.0 * kNCheb));
     const double alpha = 0.5 * r.alpha_max * (1.0 + s);
     double psi, lag;
-    geo_psi_lag(r.u, alpha, psi, lag);
-    fH[j] = psi / alpha;
-    fG[j] = lag;
-    if (j == 0) {
+    geo_psi_lag(r.u, alpha, g, psi, lag);
+    if (g == 0) { fH[j] = psi / alpha; fG[j] = lag; }
+    if (threadIdx.x < 32) {                                      // warp 0: psi at the largest visible emission angle
         double pm, lm;
-        geo_psi_lag(r.u, r.alpha_max, pm, lm);
-        A.rows[rid].psi_max = pm;
+        geo_psi_lag(r.u, r.alpha_max, g, pm, lm);
+        if (threadIdx.x == 0) A.rows[rid].psi_max = pm;
     }
+    if (threadIdx.x < 4 * kNCheb) ctab[threadIdx.x] = cospi((double)threadIdx.x / (2.0 * kNCheb));   // cos(pi m / 128), m < 256
     __syncthreads();
-    double cH = 0.0, cG = 0.0;
-    for (int i = 0; i < kNCheb; ++i) {
-        const double c = cospi((double)(j * (2 * i + 1)) / (2.0 * kNCheb));
-        cH = fma(fH[i], c, cH);
-        cG = fma(fG[i], c, cG);
+    if (threadIdx.x < 2 * kNCheb) {                              // DCT: 64 coefficients of H and of the lag
+        const int jj = threadIdx.x % kNCheb;
+        const double* fv = (threadIdx.x < kNCheb) ? fH : fG;
+        double cc = 0.0;
+        for (int i = 0; i < kNCheb; ++i) cc = fma(fv[i], ctab[(jj * (2 * i + 1)) & (4 * kNCheb - 1)], cc);
+        A.lookup[(size_t)rid * 2 * kNCheb + threadIdx.x] = cc * (2.0 / kNCheb);
     }
-    double* L = A.lookup + (size_t)rid * 2 * kNCheb;
-    L[j] = cH * (2.0 / kNCheb);
-    L[kNCheb + j] = cG * (2.0 / kNCheb);
 }
 
 // evaluate a row's lookup at given emission angles (ppm_debug_lookup)

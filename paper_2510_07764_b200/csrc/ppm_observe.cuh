@@ -35,44 +35,65 @@ __global__ void __launch_bounds__(128) k_fold(FoldArgs A)
     A.counts[((size_t)b * A.n_phase + k) * A.n_channel + c] = s;
 }
 
-// ---- K8: Poisson ln L.  One block per vector, fixed-shape tree reduction (deterministic).
-// lgamma(d+1) depends on the data only and is summed by the same kernel run with mode = 1.
-__global__ void __launch_bounds__(512) k_loglike(const double* __restrict__ counts, const double* __restrict__ data,
-                                                 const double* __restrict__ bkg, int n_phase, int n_channel,
-                                                 double exposure, const double* __restrict__ lgam_sum, int mode,
-                                                 double* __restrict__ out)
+// ---- K8: Poisson ln L (reading R14).  Two deterministic stages: kLLSplit blocks per vector reduce fixed slices of
+// the (phase, channel) plane with a fixed-shape tree; k_loglike_final adds the slice sums in index order.  Row
+// `nvec` of the partial array holds sum lgamma(d+1), which depends on the data only (blockIdx.y == nvec).
+constexpr int kLLSplit = 64;
+
+__global__ void __launch_bounds__(256) k_loglike_part(const double* __restrict__ counts, const double* __restrict__ data,
+                                                      const double* __restrict__ bkg, int n_phase, int n_channel,
+                                                      double exposure, int nvec, double* __restrict__ part,
+                                                      int* __restrict__ bad)
 {
-    __shared__ double red[512];
+    __shared__ double red[256];
     __shared__ int bad_s;
-    const int b = blockIdx.x;
+    const int b = blockIdx.y;
+    const bool lgam = (b == nvec);
     const size_t n = (size_t)n_phase * n_channel;
-    const double* C = counts + (size_t)b * n;
+    const size_t per = (n + kLLSplit - 1) / kLLSplit;
+    const size_t i0 = (size_t)blockIdx.x * per, i1 = (i0 + per < n) ? i0 + per : n;
+    const double* C = counts + (size_t)(lgam ? 0 : b) * n;
+    const double scale = exposure / n_phase;
     if (threadIdx.x == 0) bad_s = 0;
     __syncthreads();
     double s = 0.0;
-    int bad = 0;
-    for (size_t i = threadIdx.x; i < n; i += blockDim.x) {
+    int isbad = 0;
+    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
         const double d = data[i];
-        if (mode == 1) { s += lgamma(d + 1.0); continue; }
-        const int c = (int)(i % n_channel);
-        const double m = exposure * C[i] / n_phase + (bkg ? bkg[c] : 0.0);
-        if (!(m == m)) bad = 1;
+        if (lgam) { s += lgamma(d + 1.0); continue; }
+        const double m = scale * C[i] + (bkg ? bkg[i % n_channel] : 0.0);
+        if (!(m == m)) isbad = 1;
         if (d > 0.0) {
-            if (!(m > 0.0)) bad = 1; else s += d * log(m);
+            if (!(m > 0.0)) isbad = 1; else s += d * log(m);
         }
         s -= m;
     }
     red[threadIdx.x] = s;
-    if (bad) bad_s = 1;
+    if (isbad) bad_s = 1;
     __syncthreads();
-    for (int h = 256; h > 0; h >>= 1) {
+    for (int h = 128; h > 0; h >>= 1) {
         if (threadIdx.x < h) red[threadIdx.x] += red[threadIdx.x + h];
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        if (mode == 1) out[0] = red[0];
-        else out[b] = bad_s ? -INFINITY : red[0] - lgam_sum[0];
+        part[(size_t)b * kLLSplit + blockIdx.x] = red[0];
+        bad[(size_t)b * kLLSplit + blockIdx.x] = bad_s;
     }
+}
+
+__global__ void k_loglike_final(const double* __restrict__ part, const int* __restrict__ bad, int nvec,
+                                double* __restrict__ out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nvec) return;
+    double lg = 0.0, s = 0.0;
+    int isbad = 0;
+    for (int i = 0; i < kLLSplit; ++i) {
+        lg += part[(size_t)nvec * kLLSplit + i];
+        s += part[(size_t)b * kLLSplit + i];
+        isbad |= bad[(size_t)b * kLLSplit + i];
+    }
+    out[b] = isbad ? -INFINITY : s - lg;
 }
 
 // ---- FP64 peak: 8 independent DFMA chains per thread, all SMs.  flop = blocks*threads*8*iters*2.

@@ -130,3 +130,52 @@ def test_fold_and_loglike():
     # -inf when the model is zero where data are not
     ll0 = ctx.loglike(torch.zeros_like(counts), torch.as_tensor(data, device="cuda"), None, expo).cpu().numpy()
     assert np.all(np.isneginf(ll0))
+
+
+def test_c4_full_size_sampled_phases():
+    """C4 at BASELINE.json's full size (2 x 512x512 cells, 512 phases x 256 energies, N_fp = 1024) in the launch
+    configuration bench.py times; the oracle computes two of the 512 output phases."""
+    conf = gen.config_c4()
+    g, st, _ = gpu_flux(conf)
+    sel = [5, 301]
+    ref, _ = oracle_flux(conf, phase_sel=sel)
+    assert st[0] == 0 and ref.max() > 0
+    assert max_rel_err(g[0][sel], ref) <= TOL
+    assert np.all(np.isfinite(g[0])) and np.all(g[0] >= 0)
+
+
+def test_c5_loglike_parity_and_profile_counters():
+    """S0-S7 end to end on C5 vectors (cells reduced to 64x64 per spot so that the oracle runs every phase):
+    flux, folded counts and ln L against the oracle; data drawn from the ORACLE's model of vector 0."""
+    import torch
+    conf = gen.config_c5(n_vec=3, n_cells=64)
+    rsp = gen.synthetic_response(conf["energies"])
+    ctx = make_ctx(conf)
+    ctx.set_response(rsp["n_channel"], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"])
+    nph = conf["cfg"]["n_phase"]
+    oflux = [oracle_flux(conf, b)[0] for b in range(3)]
+    ocnt = [o.fold(oflux[b], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"], conf["params"][b, 5], rsp["n_channel"])
+            for b in range(3)]
+    expo = 1e6 / (ocnt[0].sum() / nph)                               # 1e6 source counts from the reference vector
+    bkg = np.full(rsp["n_channel"], 0.05 * 1e6 / (nph * rsp["n_channel"]))
+    data = np.random.default_rng(gen.SEED0 + 55).poisson(expo * ocnt[0] / nph + bkg).astype(np.float64)
+    p = torch.as_tensor(conf["params"], device="cuda")
+    ctx.profile_enable(True)
+    flux, status = ctx.evaluate(p)
+    counts = ctx.fold_response(flux, p)
+    ll = ctx.loglike(counts, torch.as_tensor(data, device="cuda"), torch.as_tensor(bkg, device="cuda"), expo)
+    prof, triples = ctx.profile_read()
+    ctx.profile_enable(False)
+    assert np.all(status.cpu().numpy() == 0)
+    fh, ch, llh = flux.cpu().numpy(), counts.cpu().numpy(), ll.cpu().numpy()
+    for b in range(3):
+        assert max_rel_err(fh[b], oflux[b]) <= TOL
+        assert max_rel_err(ch[b], ocnt[b]) <= TOL
+        ref = o.loglike(ocnt[b], data, bkg, expo)
+        assert abs(llh[b] - ref) <= 1e-9 * data.sum(), (b, llh[b], ref)
+    assert llh[0] > llh[1] and llh[0] > llh[2]                        # the data were drawn from vector 0
+    # the device-side unit counter: accumulated (cell, phase) pairs x energies; bounded by active cells x phases x energies
+    assert prof["cells"][1] == 1 and prof["cells"][0] > 0
+    nE = len(conf["energies"])
+    n_act = sum(int(ctx.debug_mask(b).sum()) for b in range(3))
+    assert 0 < triples <= n_act * nph * nE and triples % nE == 0
