@@ -419,7 +419,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         const double r = y + kMagic;
                         const int n = __double2loint(r);
                         const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        if (n >= -1000) acc[i] += val;
+                        if (n >= -1000) acc[i] += val;       // below: the exponent add wrapped, the term is 0
                     }
                 } else {
 #pragma unroll
@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         const double r = y + kMagic;
                         const int n = __double2loint(r);
                         const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        if (n >= -1000) acc[i] += val;
+                        if (n >= -1000) acc[i] += val;       // below: the exponent add wrapped, the term is 0
                     }
                 }
             }
