@@ -42,6 +42,11 @@ import gen  # noqa: E402
 FLOP_PER_TRIPLE = 86.0          # SURVEY.md 8(d) accounting constant (FMA = 2 flop)
 # nominal FP64 vector peak: 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_cells_tab launch, from the one `ncu --set full` capture of each
+# workload that has one (profiles/r1c_k_cells_tab_T_full.md); other workloads report null
+NCU_TRAFFIC_BYTES = {"T": 71.835392e6 + 53.226752e6}
+# FP64 instructions the kernel executes per triple (same capture): 16.43 DFMA + 7.11 DADD + 1.42 DMUL per warp-triple
+EXECUTED_FLOP_PER_TRIPLE = 2 * 16.43 + 7.11 + 1.42
 METRIC = "pulse-profile evaluations per second"
 UNIT = "evals/s"
 
@@ -75,7 +80,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -254,9 +259,12 @@ def main():
         step()
     sync()
     assert int(status.sum()) == 0, "workload vectors must be inside the supported domain"
+    clocks = ClockSampler(local)                   # started early: nvidia-smi needs ~0.1 s to deliver its first sample
+    for _ in range(2):
+        step()
+    sync()
     n0 = ctx.launch_count()
     ctx.profile_enable(True)
-    clocks = ClockSampler(local)
     total_ms, wall_ms, per = timed(step, args.steps)
     clk = clocks.stop()
     prof, triples = ctx.profile_read()
@@ -283,8 +291,11 @@ def main():
         except ppm.PPMError:
             peak_dfma = None
         kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
-        roofline = {"bound": "alu", "kernel": "k_cells", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
-                    "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": None,
+        table = bool(cfg["emission"])
+        roofline = {"bound": "alu", "kernel": "k_cells_tab" if table else "k_cells_bb", "achieved": achieved,
+                    "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+                    "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                    "executed_flop_per_unit": EXECUTED_FLOP_PER_TRIPLE if table else None,
                     "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
                                    "Roofline); MEASURED_PEAKS.json has no FP64 entry",
                     "peak_measured_dfma_chain": peak_dfma,
