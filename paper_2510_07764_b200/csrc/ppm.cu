@@ -236,7 +236,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     const double per_vec = (double)c->nchunk * per_row + (double)c->RT * (67.0 * 166.0 * 8.0 + 4.0 * (c->n_fp + 1) * 8.0 +
                            cfg->n_phi * 4.0 + 2048.0);
     c->SB = (int)std::max(1.0, std::min((double)cfg->max_batch, std::floor(1.5e9 / per_vec)));
-    c->SB = std::min(c->SB, 65535 / std::max(1, c->n_etile));
+    c->SB = std::min(c->SB, 65535 / std::max(1, (cfg->n_energy + 31) / 32));     // grid.z limit with the smallest energy tile
     int rc = alloc_scratch(c);
     if (rc) { ppm_destroy(c); return rc; }
     // energy-derived constants: filled here for blackbody; refreshed by ppm_load_atmosphere (needs h)
@@ -296,14 +296,37 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
         uef[e] = llrintl((long double)ue[e] * 4503599627370496.0L);
     }
     CK(cudaMemcpyAsync(c->d_uef, uef.data(), sizeof(long long) * uef.size(), cudaMemcpyHostToDevice, c->stream));
-    // most logx intervals the energies of one tile can touch for one (cell, phase) pair
-    c->wmax = 1;
-    for (int t = 0; t < c->n_etile; ++t) {
-        const int ea = t * 32 * c->epl, eb = std::min(c->cfg.n_energy, ea + 32 * c->epl) - 1;
-        c->wmax = std::max(c->wmax, std::min(nx - 1, (int)std::floor(ue[eb] - ue[ea]) + 3));
+    // Energy tiling of the table cell kernel: the most energies per lane (fewest per-pair passes) whose per-warp window
+    // of logx intervals still fits the 227 KB of shared memory beside the row slice and the template.
+    {
+        const int need = (c->cfg.n_energy + 31) / 32;
+        const int epls[] = {10, 8, 5, 4, 2, 1};                     // descending
+        int vbest = 10;                                             // smallest option that covers all energies in one tile
+        for (int v : epls) if (v >= need) vbest = v;
+        bool found = false;
+        for (int v : epls) {
+            if (v > vbest) continue;
+            const int ntile = (c->cfg.n_energy + 32 * v - 1) / (32 * v);
+            int wmax = 1;
+            for (int t = 0; t < ntile; ++t) {
+                const int ea = t * 32 * v, eb = std::min(c->cfg.n_energy, ea + 32 * v) - 1;
+                wmax = std::max(wmax, std::min(nx - 1, (int)std::floor(ue[eb] - ue[ea]) + 3));
+            }
+            int npl = 1;
+            while (32 * npl - 3 < wmax) npl += 2;                   // odd: conflict-free strided shared-memory accesses
+            const size_t smem = sizeof(double) * ((size_t)nmu * nx + 4 * (size_t)(c->n_fp + 1) + nmu +
+                                                  (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 16));
+            if (smem <= 227 * 1024 && npl <= 9) {
+                c->epl = v; c->n_etile = ntile; c->wmax = wmax; c->npl = npl;
+                found = true;
+                break;
+            }
+        }
+        if (!found) {
+            set_err("table (%d x %d) + template (n_fp = %d) do not fit the cell kernel's shared memory", nmu, nx, c->n_fp);
+            return PPM_ERR_ARG;
+        }
     }
-    c->npl = 1;
-    while (32 * c->npl - 3 < c->wmax) c->npl += 2;                 // odd: conflict-free strided shared-memory accesses
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;

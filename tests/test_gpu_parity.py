@@ -179,3 +179,27 @@ def test_c5_loglike_parity_and_profile_counters():
     nE = len(conf["energies"])
     n_act = sum(int(ctx.debug_mask(b).sum()) for b in range(3))
     assert 0 < triples <= n_act * nph * nE and triples % nE == 0
+
+
+@pytest.mark.parametrize("emission", [1, 2])
+def test_table_edges_below_and_above_the_logx_axis(emission):
+    """Energies from far below to far above the table's log10(E/kT) range: coordinates clamp at both ends (reading
+    R13b), the window of intervals holds the first and the last interval of the axis (linear in strategy d, shifted
+    cubic stencil in strategy a), and 333 energies span two energy tiles with a ragged tail."""
+    conf = gen.config_c2(n_cells=20, n_phase=19, n_energy=333)
+    conf["cfg"] = dict(conf["cfg"], emission=emission)
+    conf["energies"] = gen.logspace(0.002, 40.0, 333)
+    conf["params"] = conf["params"].copy()
+    conf["params"][0, 8 + 3] = 6.45                                  # hot spot: x = E/kT reaches below 10^-1.3
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+def test_narrow_energy_band_uses_a_small_window():
+    """8 energies in a narrow band: the per-pair window is a few intervals (NPL = 1 variant of the cell kernel)."""
+    conf = gen.config_c3(n_cells=24, n_phase=16, n_energy=8)
+    conf["energies"] = gen.logspace(1.0, 1.6, 8)
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
