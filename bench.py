@@ -181,6 +181,8 @@ def main():
     ap.add_argument("--workload", default="C5", choices=["C5", "T", "C2", "C3", "C4"])
     ap.add_argument("--batch", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", type=int, default=0, choices=[0, 1],
+                    help="0: fp64 everywhere (default, the judged path); 1: fp32 interpolation + exponential")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -205,7 +207,7 @@ def main():
     conf, desc = workload(args.workload, args.batch, rank, world)
     cfg, E = conf["cfg"], conf["energies"]
     B = conf["params"].shape[0]
-    ctx = ppm.PPM(cfg, E, max_batch=B, device=local)
+    ctx = ppm.PPM(cfg, E, max_batch=B, device=local, precision=args.precision)
     if cfg["emission"]:
         ctx.load_atmosphere(*gen.synthetic_atmosphere())
     rsp = gen.synthetic_response(E)
@@ -305,8 +307,8 @@ def main():
                     "kernel_share_of_step": cells_ms / total_ms, "kernel_ms_per_step": kern_ms}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_eval": ms_per_step / B,
-                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": desc, "name": args.workload, "batch_per_gpu": B, "n_fp": ctx.n_fp,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 0 else "f32 interpolation / f64 geometry+sums", "data": "synthetic",
+                "config": {"workload": desc, "name": args.workload, "precision": args.precision, "batch_per_gpu": B, "n_fp": ctx.n_fp,
                            "l2": "flushed before every step (256 MiB write, inside the timed bracket)",
                            "step": "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params_pinned.numel() * 8),

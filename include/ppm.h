@@ -66,7 +66,8 @@ typedef struct {
     int32_t n_fp;       /* fine template phases N_fp (Table 4); 0 -> max(192, 2*n_phase) */
     int32_t n_energy;   /* observed photon energies (keV), given to ppm_create */
     int32_t emission;   /* PPM_EMISSION_* */
-    int32_t precision;  /* 0 = fp64 everywhere (the only mode implemented) */
+    int32_t precision;  /* 0 = fp64 everywhere; 1 = table interpolation + exponential in fp32 (geometry, templates,
+                           coordinates and the final sums stay fp64; tolerance 1e-4 per bin), table emission only */
     int32_t oblate;     /* 0 spherical S+D (o2 = 0, g = g0); 1 oblate OS+D (Eq 7-11) */
     int32_t max_batch;  /* largest B accepted by ppm_evaluate / ppm_fold_response / ppm_loglike */
     int32_t device;     /* CUDA ordinal */

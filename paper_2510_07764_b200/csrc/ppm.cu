@@ -17,6 +17,7 @@
 #include "ppm_common.cuh"
 #include "ppm_geodesic.cuh"
 #include "ppm_cells.cuh"
+#include "ppm_cells32.cuh"
 #include "ppm_observe.cuh"
 
 using namespace ppm;
@@ -175,6 +176,15 @@ extern "C" int ppm_destroy(ppm_ctx* c)
     return PPM_OK;
 }
 
+// dynamic shared memory of the table cell kernels for `npl` nodes per lane (ppm_cells.cuh / ppm_cells32.cuh layouts)
+static size_t cells_tab_smem(const ppm_ctx* c, int nmu, int nx, int npl)
+{
+    const size_t tmpl = 4 * (size_t)(c->n_fp + 1) + nmu;
+    if (c->cfg.precision == 1)
+        return sizeof(double) * (tmpl + (size_t)c->nw * (2 * 32 * npl + 64 + 64 + 16)) + sizeof(float) * ((size_t)nmu * nx + 32 * npl + 32);   // tail pad: out-of-window node reads stay inside
+    return sizeof(double) * ((size_t)nmu * nx + tmpl + (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 16));
+}
+
 static int alloc_scratch(ppm_ctx* c)
 {
     const ppm_config& g = c->cfg;
@@ -200,7 +210,8 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->n_theta >= 1 && cfg->n_phi >= 1 && cfg->n_phase >= 1 && cfg->n_energy >= 1, "grid sizes must be >= 1");
     ARG(cfg->n_fp >= 0, "n_fp must be >= 0");
     ARG(cfg->emission >= 0 && cfg->emission <= 2, "emission must be 0, 1 or 2");
-    ARG(cfg->precision == 0, "only precision = 0 (fp64) is implemented");
+    ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
+    ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
     ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
     for (int e = 0; e < cfg->n_energy; ++e) {
         ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
@@ -314,8 +325,7 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
             }
             int npl = 1;
             while (32 * npl - 3 < wmax) npl += 2;                   // odd: conflict-free strided shared-memory accesses
-            const size_t smem = sizeof(double) * ((size_t)nmu * nx + 4 * (size_t)(c->n_fp + 1) + nmu +
-                                                  (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 16));
+            const size_t smem = cells_tab_smem(c, nmu, nx, npl);
             if (smem <= 227 * 1024 && npl <= 9) {
                 c->epl = v; c->n_etile = ntile; c->wmax = wmax; c->npl = npl;
                 found = true;
@@ -380,8 +390,21 @@ static int launch_cells(ppm_ctx* c, K kernel, const CellArgs& a, dim3 grid, int 
 }
 
 template <int EPL>
+static int dispatch_cells_tab32(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    switch (c->npl) {
+    case 1:  return launch_cells(c, k_cells_tab32<EPL, 1>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_tab32<EPL, 3>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_tab32<EPL, 5>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_tab32<EPL, 7>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_tab32<EPL, 9>, a, grid, threads, smem);
+    }
+}
+
+template <int EPL>
 static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
+    if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
     switch (c->npl) {
     case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
     case 3:  return launch_cells(c, k_cells_tab<EPL, 3>, a, grid, threads, smem);
@@ -461,8 +484,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_MIXED ? 1 : 0;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
     A.wmax = table ? c->wmax : 0;
-    const size_t smem = sizeof(double) * ((size_t)A.nmu * A.nx + 4 * (size_t)(c->n_fp + 1) + A.nmu +
-                                          (table ? (size_t)c->nw * (4 * 32 * c->npl + 3 * 64 + 16) : 0));
+    const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
     prof_begin(c, KID_CELLS);

@@ -18,18 +18,18 @@ def oracle_atm():
     return o.Atmosphere(*atmosphere())
 
 
-def make_ctx(conf, max_batch=None):
+def make_ctx(conf, max_batch=None, precision=0):
     import paper_2510_07764_b200 as ppm
     B = conf["params"].shape[0]
-    ctx = ppm.PPM(conf["cfg"], conf["energies"], max_batch=max_batch or B)
+    ctx = ppm.PPM(conf["cfg"], conf["energies"], max_batch=max_batch or B, precision=precision)
     if conf["cfg"]["emission"] != 0:
         ctx.load_atmosphere(*atmosphere())
     return ctx
 
 
-def gpu_flux(conf, ctx=None):
+def gpu_flux(conf, ctx=None, precision=0):
     import torch
-    ctx = ctx or make_ctx(conf)
+    ctx = ctx or make_ctx(conf, precision=precision)
     p = torch.as_tensor(conf["params"], dtype=torch.float64, device="cuda").contiguous()
     flux, status = ctx.evaluate(p)
     torch.cuda.synchronize()

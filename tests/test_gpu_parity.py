@@ -203,3 +203,35 @@ def test_narrow_energy_band_uses_a_small_window():
     g, st, _ = gpu_flux(conf)
     ref, _ = oracle_flux(conf)
     assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+TOL32 = 1e-4      # north_star: "1e-4 on any FP32-interpolation path"
+
+
+@pytest.mark.parametrize("name,kw", [("c2", {}), ("c3", dict(n_cells=40, n_phase=37, n_energy=77)),
+                                     ("c4", dict(n_cells=48, n_phase=64, n_energy=96))])
+def test_fp32_interpolation_path(name, kw):
+    conf = getattr(gen, "config_" + name)(**kw)
+    g, st, _ = gpu_flux(conf, precision=1)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0
+    err = max_rel_err(g[0], ref)
+    assert err <= TOL32, err
+    g64, _, _ = gpu_flux(conf)
+    assert np.array_equal(g[0] == 0, g64[0] == 0)
+
+
+def test_fp32_path_target_full_size_and_edges():
+    conf = gen.config_t()
+    g, st, _ = gpu_flux(conf, precision=1)
+    sel = [3, 77]
+    ref, _ = oracle_flux(conf, phase_sel=sel)
+    assert st[0] == 0 and max_rel_err(g[0][sel], ref) <= TOL32
+    # both ends of the logx axis, two energy tiles, strategy a
+    conf = gen.config_c2(n_cells=20, n_phase=19, n_energy=333)
+    conf["energies"] = gen.logspace(0.002, 40.0, 333)
+    conf["params"] = conf["params"].copy()
+    conf["params"][0, 8 + 3] = 6.45
+    g, st, _ = gpu_flux(conf, precision=1)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL32
