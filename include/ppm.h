@@ -53,6 +53,8 @@ extern "C" {
 #define PPM_EMISSION_BLACKBODY   0  /* isotropic blackbody, Eq C.5 */
 #define PPM_EMISSION_TABLE_CUBIC 1  /* 4-D table, cubic Lagrange on all axes (strategy a) */
 #define PPM_EMISSION_TABLE_MIXED 2  /* 4-D table, mixed order (strategy d) */
+#define PPM_EMISSION_TABLE_CUBIC_LINEDGE 3 /* cubic on all axes, linear at the table boundaries and in the protected
+                                             small-mu zone (strategy c; reading R13e) */
 
 #define PPM_MAX_SPOTS 4
 
@@ -65,7 +67,7 @@ typedef struct {
     int32_t n_phase;    /* output phases, phi_out[k] = k / n_phase (reading R3) */
     int32_t n_fp;       /* fine template phases N_fp (Table 4); 0 -> max(192, 2*n_phase) */
     int32_t n_energy;   /* observed photon energies (keV), given to ppm_create */
-    int32_t emission;   /* PPM_EMISSION_* */
+    int32_t emission;   /* PPM_EMISSION_* (0..3) */
     int32_t precision;  /* 0 = fp64 everywhere; 1 = table interpolation + exponential in fp32 (geometry, templates,
                            coordinates and the final sums stay fp64; tolerance 1e-4 per bin), table emission only */
     int32_t oblate;     /* 0 spherical S+D (o2 = 0, g = g0); 1 oblate OS+D (Eq 7-11) */

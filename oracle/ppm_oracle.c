@@ -586,11 +586,14 @@ double orc_interp1(const double* ax, const double* y, int n, double x, int rule)
     return v;
 }
 
-/* strategy: 1 = (a) cubic on all four axes; 2 = (d) mixed order (reading R13c) */
+/* strategy: 1 = (a) cubic on all four axes; 2 = (d) mixed order (reading R13c);
+ * 3 = (c) cubic on all four axes with linear interpolation at the table boundaries (Fig 4 caption PAPER.md:537)
+ * and in the protected small-mu zone ("linear interpolation enforced at the mu -> 0 boundary"; R13e) */
 double orc_interp4(const orc_atm* A, int strategy, double logT, double logg, double mu, double logx)
 {
     int rT, rg, rm, rx;
     if (strategy == 1) { rT = rg = rm = rx = AX_CUBIC_SHIFT; }
+    else if (strategy == 3) { rT = rg = rx = AX_CUBIC_LINEDGE; rm = AX_MU_PROTECTED; }
     else { rT = rg = AX_LINEAR; rm = AX_MU_PROTECTED; rx = AX_CUBIC_LINEDGE; }
     int bT, cT, bg, cg, bm, cm, bx, cx; double wT[4], wg[4], wm[4], wx[4];
     axis_weights(A->logT, A->nT, logT, rT, &bT, &cT, wT);

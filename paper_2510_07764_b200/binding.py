@@ -8,7 +8,7 @@ import numpy as np
 
 from . import _build
 
-EMISSION_BLACKBODY, EMISSION_TABLE_CUBIC, EMISSION_TABLE_MIXED = 0, 1, 2
+EMISSION_BLACKBODY, EMISSION_TABLE_CUBIC, EMISSION_TABLE_MIXED, EMISSION_TABLE_CUBIC_LINEDGE = 0, 1, 2, 3
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)

@@ -209,7 +209,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->n_spots >= 1 && cfg->n_spots <= PPM_MAX_SPOTS, "n_spots must be 1..4");
     ARG(cfg->n_theta >= 1 && cfg->n_phi >= 1 && cfg->n_phase >= 1 && cfg->n_energy >= 1, "grid sizes must be >= 1");
     ARG(cfg->n_fp >= 0, "n_fp must be >= 0");
-    ARG(cfg->emission >= 0 && cfg->emission <= 2, "emission must be 0, 1 or 2");
+    ARG(cfg->emission >= 0 && cfg->emission <= 3, "emission must be 0, 1, 2 or 3");
     ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
     ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
     ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
@@ -481,7 +481,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.n_fp = c->n_fp; A.nE = g.n_energy;
     A.nmu = table ? c->nmu : 0; A.nx = table ? c->nx : 0;
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
-    A.x_linedge = g.emission == PPM_EMISSION_TABLE_MIXED ? 1 : 0;
+    A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
     A.wmax = table ? c->wmax : 0;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);

@@ -234,17 +234,28 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab32(CellArgs A)
                 for (int jn = 0; jn < NPL; ++jn) K4[NPL * lane + jn] = kc[jn];
                 __syncwarp();
                 const float4* K4q = K4 + (1 - jlo);
-                const bool clamp = inf & 0x8000;
+                if (!(inf & 0x8000)) {
 #pragma unroll
-                for (int i = 0; i < EPL; ++i) {
-                    long long s = q + uef[i];
-                    if (clamp) s = s < 0 ? 0 : (s > s_top ? s_top : s);          // reading R13b (warp-uniform branch)
-                    const int shi = (int)(s >> 32);
-                    const float4 c4 = K4q[shi >> 20];
-                    // top 23 bits of the 52-bit fraction under the exponent of 1.0f: 1 + frac in FP32
-                    const float tau = __int_as_float((__funnelshift_l((int)s, shi, 3) & 0x007FFFFF) | 0x3F800000) - 1.5f;
-                    const float y = fmaf(fmaf(fmaf(c4.w, tau, c4.z), tau, c4.y), tau, c4.x) - yoff[i];
-                    acc32[i] += ex2_approx(y);
+                    for (int i = 0; i < EPL; ++i) {
+                        const long long s = q + uef[i];
+                        const int shi = (int)(s >> 32);
+                        const float4 c4 = K4q[shi >> 20];
+                        // top 23 bits of the 52-bit fraction under the exponent of 1.0f: 1 + frac in FP32
+                        const float tau = __int_as_float((__funnelshift_l((int)s, shi, 3) & 0x007FFFFF) | 0x3F800000) - 1.5f;
+                        const float y = fmaf(fmaf(fmaf(c4.w, tau, c4.z), tau, c4.y), tau, c4.x) - yoff[i];
+                        acc32[i] += ex2_approx(y);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < EPL; ++i) {
+                        long long s = q + uef[i];
+                        s = s < 0 ? 0 : (s > s_top ? s_top : s);                 // clamp to the table (reading R13b)
+                        const int shi = (int)(s >> 32);
+                        const float4 c4 = K4q[shi >> 20];
+                        const float tau = __int_as_float((__funnelshift_l((int)s, shi, 3) & 0x007FFFFF) | 0x3F800000) - 1.5f;
+                        const float y = fmaf(fmaf(fmaf(c4.w, tau, c4.z), tau, c4.y), tau, c4.x) - yoff[i];
+                        acc32[i] += ex2_approx(y);
+                    }
                 }
             }
             // flush the batch's FP32 sums into the FP64 accumulators (exact power-of-two scaling)

@@ -101,6 +101,13 @@ __device__ inline void cheb_eval(const double* __restrict__ c, double s, double&
 // ------------------------------------------------------------------------------------------------
 // K0: per vector -- star scalars (Eq 7-8, 11), domain check (reading R4), per-spot box and T stencil.
 // ------------------------------------------------------------------------------------------------
+// rule of the log T and log g axes per emission mode (strategies a, d, c; readings R13c, R13e)
+__host__ __device__ inline int tg_rule(int emission)
+{
+    return emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT
+         : emission == PPM_EMISSION_TABLE_CUBIC_LINEDGE ? AX_CUBIC_LINEDGE : AX_LINEAR;
+}
+
 struct GeoArgs {
     const double* params;   // [nb][P]
     int nb, P, n_spots, n_theta, n_phi, n_phase, n_fp, oblate, emission;
@@ -168,7 +175,7 @@ __global__ void k_star(GeoArgs A)
         sp.bT = 0; sp.pad = 0;
         sp.wT[0] = sp.wT[1] = sp.wT[2] = sp.wT[3] = 0.0;
         if (A.emission != PPM_EMISSION_BLACKBODY && !status)
-            axis_w4(A.axT, A.nT, sp.log10T, A.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_LINEAR,
+            axis_w4(A.axT, A.nT, sp.log10T, tg_rule(A.emission),
                     sp.bT, sp.wT);
         A.spots[(size_t)b * A.n_spots + j] = sp;
     }
@@ -221,7 +228,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         r.psi_max = 0.0;
         r.bg = 0; r.wg[0] = r.wg[1] = r.wg[2] = r.wg[3] = 0.0;
         if (A.emission != PPM_EMISSION_BLACKBODY && !st.status)
-            axis_w4(A.axg, A.ng, r.log10g, A.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_LINEAR,
+            axis_w4(A.axg, A.ng, r.log10g, tg_rule(A.emission),
                     r.bg, r.wg);
         r.n_active = 0; r.visible = 0; r.pad = 0;
         row = r;

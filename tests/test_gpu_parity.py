@@ -235,3 +235,16 @@ def test_fp32_path_target_full_size_and_edges():
     g, st, _ = gpu_flux(conf, precision=1)
     ref, _ = oracle_flux(conf)
     assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL32
+
+
+def test_strategy_c_cubic_with_linear_edges():
+    """emission = 3 (strategy c): C3's cool ring sits in the first logT intervals (linear there),
+    the hot cap in the interior (cubic in logT and logg)."""
+    conf = gen.config_c3(n_cells=32, n_phase=24, n_energy=70)
+    conf["cfg"] = dict(conf["cfg"], emission=3)
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+    conf2 = dict(conf, cfg=dict(conf["cfg"], emission=2))
+    g2, _, _ = gpu_flux(conf2)
+    assert np.max(np.abs(g2[0] - g[0]) / np.maximum(g[0], 1e-300)) > 1e-7      # and it differs from strategy d

@@ -32,7 +32,7 @@ def _random_points(n, seed=1, inside_only=False):
     return pts
 
 
-@pytest.mark.parametrize("strategy", [1, 2])
+@pytest.mark.parametrize("strategy", [1, 2, 3])
 def test_p11_reproduces_nodes(strategy):
     logT, logg, mu, logx, vals = gen.synthetic_atmosphere()
     atm = o.Atmosphere(logT, logg, mu, logx, vals)
@@ -81,11 +81,41 @@ def test_p11_strategy_d_local_orders():
     assert abs(o.interp4(atmT, 2, *p) - fT(*p)) > 1e-7
 
 
+def test_p11_strategy_c_local_orders():
+    """(c) (PAPER.md:537 caption, 551; reading R13e): cubic on all four axes in the interior; linear in the first / last
+    interval of logT, logg, logx, for mu <= mu[3] and in the last mu interval."""
+    logT, logg, mu, logx = _axes()
+    atm, f = _poly_table(3, 3, 3, 3)
+    rng = np.random.default_rng(5)
+    for _ in range(300):                                     # interior of every axis: exact for tensor cubics
+        p = [rng.uniform(logT[1], logT[-2]), rng.uniform(logg[1], logg[-2]),
+             rng.uniform(mu[3], mu[-2]), rng.uniform(logx[1], logx[-2])]
+        assert abs(o.interp4(atm, 3, *p) - f(*p)) < 1e-11
+    atm1, f1 = _poly_table(1, 1, 1, 1)
+    for _ in range(200):                                     # everywhere: exact for multilinear
+        p = _random_points(1, seed=int(rng.integers(1 << 30)))[0]
+        assert abs(o.interp4(atm1, 3, *p) - f1(*p)) < 1e-12
+    # first logT interval: linear between the two nodes, not the cubic
+    atmT, fT = _poly_table(3, 0, 0, 0)
+    tm = 0.5 * (logT[0] + logT[1])
+    lin = 0.5 * (fT(logT[0], 14.2, 0.5, 0.3) + fT(logT[1], 14.2, 0.5, 0.3))
+    assert abs(o.interp4(atmT, 3, tm, 14.2, 0.5, 0.3) - lin) < 1e-13
+    assert abs(o.interp4(atmT, 3, tm, 14.2, 0.5, 0.3) - fT(tm, 14.2, 0.5, 0.3)) > 1e-9
+    # interior logT: (c) agrees with (a), differs from (d)
+    p = [5.93, 14.2, 0.5, 0.3]
+    assert abs(o.interp4(atmT, 3, *p) - o.interp4(atmT, 1, *p)) < 1e-13
+    assert abs(o.interp4(atmT, 3, *p) - o.interp4(atmT, 2, *p)) > 1e-7
+    # protected small-mu zone as in (d)
+    atm3, f3 = _poly_table(0, 0, 3, 0)
+    q = [6.0, 14.2, 0.5 * (mu[1] + mu[2]), 0.3]
+    assert abs(o.interp4(atm3, 3, *q) - o.interp4(atm3, 2, *q)) < 1e-13
+
+
 def test_p11_continuity_across_nodes_and_zone_boundary():
     logT, logg, mu, logx, vals = gen.synthetic_atmosphere()
     atm = o.Atmosphere(logT, logg, mu, logx, vals)
     eps = 1e-10
-    for strategy in (1, 2):
+    for strategy in (1, 2, 3):
         for k in (1, 2, 3, 4, 30, 65):                       # mu nodes incl. the protected-zone edge mu[3]
             a = o.interp4(atm, strategy, 6.03, 14.21, mu[k] - eps, 0.77)
             b = o.interp4(atm, strategy, 6.03, 14.21, mu[k] + eps, 0.77)
