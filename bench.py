@@ -72,8 +72,10 @@ def workload(name, batch, rank, world=1):
 
 
 class ClockSampler:
-    """nvidia-smi clock / throttle-reason samples during the timed region (profiling recipe)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clock / throttle-reason samples (profiling recipe).  Started at process start (nvidia-smi needs a few
+    hundred ms to deliver its first line); stop(t0, t1) keeps the samples whose timestamp falls inside the timed
+    region [t0, t1] (time.time() values), or, for regions shorter than the sampling period, the nearest sample."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -81,15 +83,17 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
-    def stop(self):
+    def stop(self, t0, t1):
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.p is None:
             return out
+        time.sleep(0.05)
         self.p.terminate()
         try:
             self.p.wait(timeout=5)
@@ -97,24 +101,27 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, smax, pw, reasons = [], [], [], set()
+        rows = []
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
         for line in self.f:
             c = [x.strip() for x in line.split(",")]
-            if len(c) < 7:
+            if len(c) < 8:
                 continue
             try:
-                sm.append(float(c[0])); smax.append(float(c[1])); pw.append(float(c[2]))
+                ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(c[1]), float(c[2]), float(c[3]),
+                             [n for n, v in zip(names, c[4:8]) if v.lower().startswith("active")]))
             except ValueError:
                 continue
-            for n, v in zip(names, c[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
         self.f.close()
         os.unlink(self.f.name)
-        if sm:
-            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), reasons=sorted(reasons),
-                       samples=len(sm), power_w_max=max(pw))
+        inside = [r for r in rows if t0 <= r[0] <= t1]
+        if not inside and rows:
+            inside = [min(rows, key=lambda r: abs(r[0] - 0.5 * (t0 + t1)))]
+        if inside:
+            out.update(sm_mhz=statistics.median(r[1] for r in inside), sm_max_mhz=max(r[2] for r in inside),
+                       reasons=sorted({n for r in inside for n in r[4]}), samples=len(inside),
+                       power_w_max=max(r[3] for r in inside))
         return out
 
 
@@ -192,6 +199,7 @@ def main():
         run_reference(args, rank)
         return
     args.warmup = max(args.warmup, 3)
+    clocks = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
 
     import torch
     import paper_2510_07764_b200 as ppm
@@ -262,14 +270,11 @@ def main():
         step()
     sync()
     assert int(status.sum()) == 0, "workload vectors must be inside the supported domain"
-    clocks = ClockSampler(local)                   # started early: nvidia-smi needs ~0.1 s to deliver its first sample
-    for _ in range(2):
-        step()
-    sync()
     n0 = ctx.launch_count()
     ctx.profile_enable(True)
+    t_begin = time.time()
     total_ms, wall_ms, per = timed(step, args.steps)
-    clk = clocks.stop()
+    clk = clocks.stop(t_begin, time.time())
     prof, triples = ctx.profile_read()
     ctx.profile_enable(False)
     launches = ctx.launch_count() - n0

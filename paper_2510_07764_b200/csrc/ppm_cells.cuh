@@ -397,6 +397,12 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         }
                     }
                 }
+                // terms below 2^-900 (possible only with extreme table values) take the guarded loop: the exponent add of
+                // exp2_frac_scaled must not wrap.  k0 is the exponent at the interval midpoint; +-100 covers the interval.
+                bool tiny = false;
+#pragma unroll
+                for (int jn = 0; jn < NPL; ++jn) tiny |= (n0 + jn >= jlo) && (n0 + jn <= jhi) && !(ka[jn].x > -800.0);
+                const bool guarded = __any_sync(0xffffffffu, tiny) || (inf & 0x8000);
                 __syncwarp();                                                   // the previous pair's readers are done
 #pragma unroll
                 for (int jn = 0; jn < NPL; ++jn) {
@@ -406,7 +412,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 __syncwarp();
                 const double2* KAq = KA + (1 - jlo);
                 // ---- energies ----
-                if (!(inf & 0x8000)) {
+                if (!guarded) {
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
                         const long long s = q + uef[i];
@@ -418,7 +424,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         const double r = y + kMagic;
                         const int n = __double2loint(r);
                         const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        if (n >= -1000) acc[i] += val;       // below: the exponent add wrapped, the term is 0
+                        acc[i] += val;
                     }
                 } else {
 #pragma unroll

@@ -248,3 +248,26 @@ def test_strategy_c_cubic_with_linear_edges():
     conf2 = dict(conf, cfg=dict(conf["cfg"], emission=2))
     g2, _, _ = gpu_flux(conf2)
     assert np.max(np.abs(g2[0] - g[0]) / np.maximum(g[0], 1e-300)) > 1e-7      # and it differs from strategy d
+
+
+def test_terms_that_underflow_take_the_guarded_loop():
+    """A table whose high-x half lies 300 decades lower: there F_p T^3 10^v < 2^-1000, the exponent add of the fast
+    2^y would wrap; such pairs must take the guarded loop and contribute (numerically) nothing, and the bins the
+    oracle resolves as normal numbers must still agree to 1e-9."""
+    import oracle as orc
+    import paper_2510_07764_b200 as ppm
+    import torch
+    logT, logg, mu, logx, vals = gen.synthetic_atmosphere()
+    vals = vals.copy()
+    vals[..., 120:] -= 300.0
+    conf = gen.config_c3(n_cells=24, n_phase=16, n_energy=60)
+    ctx = ppm.PPM(conf["cfg"], conf["energies"], max_batch=1)
+    ctx.load_atmosphere(logT, logg, mu, logx, vals)
+    flux, st = ctx.evaluate(torch.as_tensor(conf["params"], device="cuda"))
+    g = flux.cpu().numpy()[0]
+    ref, _ = orc.evaluate(conf["cfg"], conf["energies"], conf["params"][0], orc.Atmosphere(logT, logg, mu, logx, vals))
+    assert int(st[0]) == 0 and np.all(np.isfinite(g)) and np.all(g >= 0)
+    big = ref > 1e-250
+    assert big.any() and (~big).any()
+    assert np.max(np.abs(g[big] - ref[big]) / ref[big]) <= TOL
+    assert np.all(g[~big] <= 1e-240)
