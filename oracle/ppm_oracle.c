@@ -388,13 +388,20 @@ void orc_spot_box(const orc_spot* sp, int n_theta, int n_phi, orc_box* bx)
     bx->dphi = 2.0 * bx->W / n_phi;
 }
 
+static void row_from_theta(const orc_star* s, double th, double dcos, orc_row* r);
+
 void orc_row_init(const orc_star* s, const orc_box* bx, int n_theta, int j, orc_row* r)
 {
     double e0 = bx->theta_lo + (bx->theta_hi - bx->theta_lo) * (double)j / n_theta;
     double e1 = bx->theta_lo + (bx->theta_hi - bx->theta_lo) * (double)(j + 1) / n_theta;
-    double th = 0.5 * (e0 + e1);
+    row_from_theta(s, 0.5 * (e0 + e1), cos(e0) - cos(e1), r);
+}
+
+/* row scalars at colatitude th (Eq 2-3, 7, 10-11, 16, 18) */
+static void row_from_theta(const orc_star* s, double th, double dcos, orc_row* r)
+{
     r->theta = th;
-    r->dcos = cos(e0) - cos(e1);
+    r->dcos = dcos;
     double ct = cos(th), st = sin(th);
     double R = s->Re_cm * (1.0 + s->o2 * ct * ct);               /* Eq 7 */
     double u = s->Rs_cm / R;
@@ -407,6 +414,34 @@ void orc_row_init(const orc_star* s, const orc_box* bx, int n_theta, int j, orc_
     r->gamma = 1.0 / sqrt(1.0 - r->beta * r->beta);
     r->log10g = log10(s->g0_cgs * g_ratio(s, th));               /* Eq 10-11 */
     r->c_dt_cm = (double)c_delta_t((ld)s->Re_cm, (ld)s->Rs_cm, (ld)R);    /* Eq 16 */
+}
+
+/* HEALPix ring scheme (Eq 24-29): ring i = 1 .. 4 N_side - 1 -> cos(theta) of its pixel centres,
+ * number of pixels, azimuth of pixel i_phi = 1 and azimuth step; every pixel covers pi / (3 N_side^2) sr. */
+void orc_healpix_ring(int nside, int i, double* costheta, int* npix, double* phi0, double* dphi)
+{
+    int south = i > 2 * nside;
+    int in = south ? 4 * nside - i : i;                           /* Eq 28-29: mirror of the northern ring */
+    double z;
+    if (in < nside) {                                             /* Eq 24-25 */
+        z = 1.0 - (double)in * (double)in / (3.0 * (double)nside * (double)nside);
+        *npix = 4 * in;
+        *dphi = M_PI / (2.0 * (double)in);
+        *phi0 = *dphi * 0.5;
+    } else {                                                      /* Eq 26-27 */
+        z = 4.0 / 3.0 - 2.0 * (double)in / (3.0 * (double)nside);
+        *npix = 4 * nside;
+        *dphi = M_PI / (2.0 * (double)nside);
+        *phi0 = *dphi * (1.0 - 0.5 * (double)((in - nside + 1) % 2));
+    }
+    *costheta = south ? -z : z;
+}
+
+void orc_row_init_healpix(const orc_star* s, int nside, int j, orc_row* r)
+{
+    double z, phi0, dphi; int npix;
+    orc_healpix_ring(nside, j + 1, &z, &npix, &phi0, &dphi);
+    row_from_theta(s, acos(z), M_PI / (3.0 * (double)nside * (double)nside) / dphi, r);   /* dcos := dOmega / dphi */
 }
 
 /* cell (j,m) active?  centre-in test for the cap, minus the omitted (masking) cap
@@ -440,6 +475,24 @@ int orc_spot_mask(const orc_spot* sp, int n_theta, int n_phi, uint8_t* mask)
         double th = 0.5 * (e0 + e1);
         for (int m = 0; m < n_phi; ++m) {
             int a = cell_active(sp, th, cell_dphi(&bx, m));
+            mask[(size_t)j * n_phi + m] = (uint8_t)a; n += a;
+        }
+    }
+    return n;
+}
+
+/* HEALPix mask[4 nside - 1][4 nside] (1 = active; entries beyond a ring's pixel count are 0) */
+int orc_spot_mask_healpix(const orc_spot* sp, int nside, uint8_t* mask)
+{
+    int n = 0;
+    const int n_phi = 4 * nside;
+    memset(mask, 0, (size_t)(4 * nside - 1) * n_phi);
+    for (int j = 0; j < 4 * nside - 1; ++j) {
+        double z, phi0, dphi; int npix;
+        orc_healpix_ring(nside, j + 1, &z, &npix, &phi0, &dphi);
+        double th = acos(z);
+        for (int m = 0; m < npix; ++m) {
+            int a = cell_active(sp, th, (phi0 + (double)m * dphi) - sp->phi_c);
             mask[(size_t)j * n_phi + m] = (uint8_t)a; n += a;
         }
     }
@@ -639,6 +692,8 @@ double orc_intensity(int emission, const orc_atm* A, double log10T, double log10
  * ---------------------------------------------------------------------------------- */
 typedef struct {
     int32_t n_spots, n_theta, n_phi, n_phase, n_fp, n_energy, emission, oblate;
+    int32_t mesh;    /* 0: per-spot theta x phi bounding-box grid (reading R1); 1: HEALPix rings (Eq 24-29) with
+                        N_side = n_phi / 4, n_theta = 4 N_side - 1, the same mesh for every spot */
 } orc_config;
 
 #define ORC_U_MAX 0.560     /* supported compactness domain (reading R4) */
@@ -691,18 +746,31 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
             const double* q = params + 8 + 8 * sidx;
             orc_spot sp = { q[0], q[1], q[2], q[3], q[4], q[5], q[6] };
             orc_box bx; orc_spot_box(&sp, cfg->n_theta, cfg->n_phi, &bx);
-            orc_row row; orc_row_init(&star, &bx, cfg->n_theta, j, &row);
+            orc_row row;
+            int npix = cfg->n_phi;
+            double hp_phi0 = 0.0, hp_dphi = 0.0, dOmega;
+            if (cfg->mesh == 1) {
+                const int nside = cfg->n_phi / 4;
+                double zc;
+                orc_healpix_ring(nside, j + 1, &zc, &npix, &hp_phi0, &hp_dphi);
+                orc_row_init_healpix(&star, nside, j, &row);
+                dOmega = M_PI / (3.0 * (double)nside * (double)nside);      /* PAPER.md:306 */
+            } else {
+                orc_row_init(&star, &bx, cfg->n_theta, j, &row);
+                dOmega = row.dcos * bx.dphi;
+            }
+#define CELL_DPHI(m) (cfg->mesh == 1 ? (hp_phi0 + (double)(m) * hp_dphi) - sp.phi_c : cell_dphi(&bx, (m)))
             /* active azimuths of this ring (PAPER.md:372) */
             int n_act = 0;
-            for (int m = 0; m < cfg->n_phi; ++m) n_act += cell_active(&sp, row.theta, cell_dphi(&bx, m));
+            for (int m = 0; m < npix; ++m) n_act += cell_active(&sp, row.theta, CELL_DPHI(m));
             if (n_act == 0) continue;
             double mg;
-            int visible = orc_template(&star, &row, cosi, D_cm, row.dcos * bx.dphi, nfp, F, z, po, mu, NULL, &mg, NULL, NULL);
+            int visible = orc_template(&star, &row, cosi, D_cm, dOmega, nfp, F, z, po, mu, NULL, &mg, NULL, NULL);
             if (mg < margin_thr) margin_thr = mg;
             if (!visible) continue;
             /* O5 shift-and-add (PAPER.md:417-430) */
-            for (int m = 0; m < cfg->n_phi; ++m) {
-                double dphi_m = cell_dphi(&bx, m);
+            for (int m = 0; m < npix; ++m) {
+                double dphi_m = CELL_DPHI(m);
                 if (!cell_active(&sp, row.theta, dphi_m)) continue;
                 double phi_m = sp.phi_c + dphi_m;
                 for (int kk = 0; kk < nk; ++kk) {

@@ -44,7 +44,8 @@ class _Atm(C.Structure):
 
 class _Config(C.Structure):
     _fields_ = [("n_spots", C.c_int32), ("n_theta", C.c_int32), ("n_phi", C.c_int32), ("n_phase", C.c_int32),
-                ("n_fp", C.c_int32), ("n_energy", C.c_int32), ("emission", C.c_int32), ("oblate", C.c_int32)]
+                ("n_fp", C.c_int32), ("n_energy", C.c_int32), ("emission", C.c_int32), ("oblate", C.c_int32),
+                ("mesh", C.c_int32)]
 
 
 def _sig(name, res, args):
@@ -78,6 +79,9 @@ _evaluate = _sig("orc_evaluate", C.c_int,
                  [C.POINTER(_Config), _dp, _dp, C.POINTER(_Atm), _ip, C.c_int, _dp, _dp])
 _fold = _sig("orc_fold", None, [_dp, C.c_int, C.c_int, C.c_int, C.c_int, _ip, _dp, _dp, C.c_double, _dp])
 _loglike = _sig("orc_loglike", C.c_double, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double])
+_hp_ring = _sig("orc_healpix_ring", None, [C.c_int, C.c_int, _dp, C.POINTER(C.c_int), _dp, _dp])
+_hp_mask = _sig("orc_spot_mask_healpix", C.c_int, [C.POINTER(Spot), C.c_int, _u8p])
+_hp_row = _sig("orc_row_init_healpix", None, [C.POINTER(Star), C.c_int, C.c_int, C.POINTER(Row)])
 _chi2 = _sig("orc_chi2", C.c_double, [_dp, _dp, C.c_size_t])
 _nthreads = _sig("orc_num_threads", C.c_int, [])
 _set_nthreads = _sig("orc_set_num_threads", None, [C.c_int])
@@ -182,6 +186,26 @@ def spot_mask(sp, n_theta, n_phi):
     return m
 
 
+def healpix_ring(nside, i):
+    """Ring i = 1 .. 4 nside - 1 of the HEALPix ring scheme (Eq 24-29): -> (cos theta, npix, phi of pixel 1, dphi)."""
+    z, p0, dp = C.c_double(), C.c_double(), C.c_double()
+    n = C.c_int()
+    _hp_ring(int(nside), int(i), C.byref(z), C.byref(n), C.byref(p0), C.byref(dp))
+    return z.value, n.value, p0.value, dp.value
+
+
+def spot_mask_healpix(sp, nside):
+    m = np.zeros((4 * nside - 1, 4 * nside), dtype=np.uint8)
+    _hp_mask(C.byref(sp), int(nside), m.ctypes.data_as(_u8p))
+    return m
+
+
+def row_healpix(st, nside, j):
+    r = Row()
+    _hp_row(C.byref(st), int(nside), int(j), C.byref(r))
+    return r
+
+
 def template(st, rw, cosi, D_cm, dOmega, n_fp):
     """Ring template (O3+O4).  Returns dict(F, z, phio, mu, vis, margin, alpha, lf, visible)."""
     F, z, po, mu, al, lf = (np.zeros(n_fp + 1) for _ in range(6))
@@ -225,7 +249,7 @@ def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=Fals
     energies = _f64(energies)
     params = _f64(params)
     c = _Config(cfg["n_spots"], cfg["n_theta"], cfg["n_phi"], cfg["n_phase"], cfg["n_fp"],
-                len(energies), cfg["emission"], int(cfg.get("oblate", 1)))
+                len(energies), cfg["emission"], int(cfg.get("oblate", 1)), int(cfg.get("mesh", 0)))
     assert params.shape == (8 + 8 * cfg["n_spots"],)
     if cfg["emission"] != 0:
         assert atm is not None

@@ -105,7 +105,7 @@ struct ppm_ctx {
     int64_t launches = 0;
     int last_nb = 0;
     // energy grid
-    double *d_en = nullptr, *d_ue = nullptr, *d_le2 = nullptr;
+    double* d_en = nullptr;
     long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
     int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
     std::vector<double> h_en;
@@ -122,7 +122,6 @@ struct ppm_ctx {
     // scratch (sub-batch sized)
     StarD* d_stars = nullptr; SpotD* d_spots = nullptr; RowD* d_rows = nullptr; int* d_cells = nullptr;
     double *d_lookup = nullptr, *d_tmpl = nullptr, *d_slices = nullptr, *d_partial = nullptr;
-    double* d_lgam = nullptr;
     double* d_llpart = nullptr; int* d_llbad = nullptr; int llpart_cap = 0;   // ln L slice sums [cap][kLLSplit]
     // host-variant staging
     double *d_params_stage = nullptr, *d_flux_stage = nullptr, *d_ll_stage = nullptr, *d_counts_stage = nullptr;
@@ -163,9 +162,9 @@ extern "C" int ppm_destroy(ppm_ctx* c)
 {
     if (!c) return PPM_OK;
     cudaSetDevice(c->cfg.device);
-    void* ptrs[] = {c->d_en, c->d_ue, c->d_le2, c->d_uef, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
+    void* ptrs[] = {c->d_en, c->d_uef, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
                     c->d_ehi, c->d_band, c->d_tau, c->d_stars, c->d_spots, c->d_rows, c->d_cells, c->d_lookup,
-                    c->d_tmpl, c->d_slices, c->d_partial, c->d_lgam, c->d_params_stage, c->d_flux_stage,
+                    c->d_tmpl, c->d_slices, c->d_partial, c->d_params_stage, c->d_flux_stage,
                     c->d_ll_stage, c->d_counts_stage, c->d_status_stage};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (c->d_pairs) cudaFree(c->d_pairs);
@@ -197,7 +196,6 @@ static int alloc_scratch(ppm_ctx* c)
     if ((rc = dev_alloc(&c->d_lookup, rows * 2 * kNCheb))) return rc;
     if ((rc = dev_alloc(&c->d_tmpl, rows * 4 * (c->n_fp + 1)))) return rc;
     if ((rc = dev_alloc(&c->d_partial, (size_t)c->SB * c->nchunk * g.n_phase * g.n_energy))) return rc;
-    if ((rc = dev_alloc(&c->d_lgam, (size_t)1))) return rc;
     if ((rc = dev_alloc(&c->d_pairs, (size_t)1))) return rc;
     if (cudaMemsetAsync(c->d_pairs, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return PPM_ERR_CUDA;
     return PPM_OK;
@@ -251,13 +249,11 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     int rc = alloc_scratch(c);
     if (rc) { ppm_destroy(c); return rc; }
     // energy-derived constants: filled here for blackbody; refreshed by ppm_load_atmosphere (needs h)
-    if ((rc = dev_alloc(&c->d_en, (size_t)cfg->n_energy)) || (rc = dev_alloc(&c->d_ue, (size_t)cfg->n_energy)) ||
-        (rc = dev_alloc(&c->d_uef, (size_t)cfg->n_energy)) ||
-        (rc = dev_alloc(&c->d_le2, (size_t)cfg->n_energy))) { ppm_destroy(c); return rc; }
-    std::vector<double> le2(cfg->n_energy);
-    for (int e = 0; e < cfg->n_energy; ++e) le2[e] = -std::log2(energies[e]);
+    if ((rc = dev_alloc(&c->d_en, (size_t)cfg->n_energy)) || (rc = dev_alloc(&c->d_uef, (size_t)cfg->n_energy))) {
+        ppm_destroy(c);
+        return rc;
+    }
     CK(cudaMemcpyAsync(c->d_en, energies, sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->d_le2, le2.data(), sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream));
     double glx[kNGL], glw[kNGL];
     gauss_legendre(kNGL, glx, glw);
     CK(cudaMemcpyToSymbolAsync(c_glx, glx, sizeof(glx), 0, cudaMemcpyHostToDevice, c->stream));
@@ -300,7 +296,6 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     c->nT = nT; c->ng = ng; c->nmu = nmu; c->nx = nx; c->x0 = logx[0]; c->hx = h;
     std::vector<double> ue(c->cfg.n_energy);
     for (int e = 0; e < c->cfg.n_energy; ++e) ue[e] = std::log10(c->h_en[e]) / h;
-    CK(cudaMemcpyAsync(c->d_ue, ue.data(), sizeof(double) * ue.size(), cudaMemcpyHostToDevice, c->stream));
     std::vector<long long> uef(c->cfg.n_energy);
     for (int e = 0; e < c->cfg.n_energy; ++e) {
         ARG(std::fabs(ue[e]) < 1000.0, "energies are too far outside the table's log10(E/kT) range");
@@ -474,7 +469,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     }
     CellArgs A;
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
-    A.slices = c->d_slices; A.axmu = c->d_axmu; A.ue = c->d_ue; A.uef = c->d_uef; A.le2 = c->d_le2; A.en = c->d_en;
+    A.slices = c->d_slices; A.axmu = c->d_axmu; A.uef = c->d_uef; A.en = c->d_en;
     A.partial = c->d_partial; A.pairs = c->d_pairs;
     A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;
@@ -483,7 +478,6 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
-    A.wmax = table ? c->wmax : 0;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);

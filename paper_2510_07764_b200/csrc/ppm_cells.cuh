@@ -13,9 +13,8 @@ struct CellArgs {
     const double* tmpl;      // [rows][4][n_fp+1]
     const double* slices;    // [rows][nmu][nx]  (table emission)
     const double* axmu;      // [nmu]
-    const double* ue;        // [nE]: log10(E_e) / h   (h = logx spacing)
-    const long long* uef;    // [nE]: round(ue * 2^52): the same in fixed point (units of 2^-52 intervals)
-    const double* le2;       // [nE]: -log2(E_e)
+    const long long* uef;    // [nE]: round(log10(E_e) / h * 2^52): energy part of the logx coordinate in fixed point
+                             //       (h = logx spacing; units of 2^-52 table intervals)
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
     unsigned long long* pairs;   // counter: (cell, phase) pairs with F_p != 0 (energy tile 0 only)
@@ -23,7 +22,6 @@ struct CellArgs {
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
     int nchunk, rows_per_chunk, nw, n_etile;
-    int wmax;                // table path: most logx intervals one (pair, energy tile) can touch
 };
 
 // ---- K4: collapse the 4-D table to the row's (mu x logx) slice: T is per spot, g per row -------
