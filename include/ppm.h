@@ -73,6 +73,9 @@ typedef struct {
     int32_t oblate;     /* 0 spherical S+D (o2 = 0, g = g0); 1 oblate OS+D (Eq 7-11) */
     int32_t max_batch;  /* largest B accepted by ppm_evaluate / ppm_fold_response / ppm_loglike */
     int32_t device;     /* CUDA ordinal */
+    int32_t mesh;       /* 0: per-spot colatitude x azimuth bounding-box grid (reading R1);
+                           1: HEALPix ring scheme over the whole surface (Eq 24-29), the same mesh
+                              for every spot: n_phi = 4 N_side, n_theta = 4 N_side - 1 rings, pixel area pi/(3 N_side^2) */
 } ppm_config;
 
 /* Create a context: copies the energy grid (host, [n_energy], keV, strictly increasing),

@@ -211,6 +211,9 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
     ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
     ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
+    ARG(cfg->mesh == 0 || cfg->mesh == 1, "mesh must be 0 (theta x phi box per spot) or 1 (HEALPix rings)");
+    ARG(cfg->mesh == 0 || (cfg->n_phi % 4 == 0 && cfg->n_theta == cfg->n_phi - 1),
+        "HEALPix mesh: n_phi = 4 N_side and n_theta = 4 N_side - 1");
     for (int e = 0; e < cfg->n_energy; ++e) {
         ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
         if (e) ARG(energies[e] > energies[e - 1], "energies must be strictly increasing");
@@ -437,7 +440,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     const bool table = g.emission != PPM_EMISSION_BLACKBODY;
     GeoArgs G;
     G.params = params_dev; G.nb = nb; G.P = c->P; G.n_spots = g.n_spots; G.n_theta = g.n_theta; G.n_phi = g.n_phi;
-    G.n_phase = g.n_phase; G.n_fp = c->n_fp; G.oblate = g.oblate; G.emission = g.emission;
+    G.n_phase = g.n_phase; G.n_fp = c->n_fp; G.oblate = g.oblate; G.emission = g.emission; G.mesh = g.mesh;
     G.stars = c->d_stars; G.spots = c->d_spots; G.rows = c->d_rows; G.cells = c->d_cells;
     G.lookup = c->d_lookup; G.tmpl = c->d_tmpl;
     G.axT = c->d_axT; G.nT = c->nT; G.axg = c->d_axg; G.ng = c->ng;
@@ -477,7 +480,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.nmu = table ? c->nmu : 0; A.nx = table ? c->nx : 0;
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
-    A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile;
+    A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);

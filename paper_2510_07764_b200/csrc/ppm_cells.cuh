@@ -21,7 +21,7 @@ struct CellArgs {
     double x0_over_h, inv_h;
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
-    int nchunk, rows_per_chunk, nw, n_etile;
+    int nchunk, rows_per_chunk, nw, n_etile, mesh;
 };
 
 // ---- K4: collapse the 4-D table to the row's (mu x logx) slice: T is per spot, g per row -------
@@ -130,8 +130,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
             double Fp = 0.0, pa = 0.0, pb = 0.0;      // pa = z_p / kT, pb = F_p z_p^3 2/(h^3 c^2)
             if (idx < nact) {
                 const int m = cl[idx];
-                const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
-                const double phi_m = sp.phi_c + dphi_m;
+                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
                 const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
                 const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
                 int lo = 0, hi = A.n_fp;
@@ -306,8 +305,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
             int info = 0;                             // slice offset of the mu stencil's first row | jlo << 16 | jhi << 24
             if (idx < nact) {
                 const int m = cl[idx];
-                const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
-                const double phi_m = sp.phi_c + dphi_m;
+                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
                 const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
                 const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
                 int lo = 0, hi = A.n_fp;

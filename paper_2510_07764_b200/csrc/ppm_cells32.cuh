@@ -147,8 +147,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab32(CellArgs A)
             int info = 0;
             if (idx < nact) {
                 const int m = cl[idx];
-                const double dphi_m = -sp.W + ((double)m + 0.5) * sp.dphi;
-                const double phi_m = sp.phi_c + dphi_m;
+                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
                 const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
                 const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
                 int lo = 0, hi = A.n_fp;

@@ -46,7 +46,8 @@ struct RowD {
     double theta, dcos, R, u, f, coseta, sineta, beta, gamma, log10g, c_dt, dOmega;
     double alpha_max, psi_max;
     double wg[4];                                 // log g axis stencil
-    int bg, n_active, visible, pad;
+    int bg, n_active, visible, npix;              // npix: azimuth cells of this row (HEALPix rings differ)
+    double phi0, dphi;                            // azimuth of cell m: phi0 + m dphi (HEALPix mesh only)
 };
 
 __host__ __device__ inline int imin_(int a, int b) { return a < b ? a : b; }

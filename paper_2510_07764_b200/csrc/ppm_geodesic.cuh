@@ -110,7 +110,7 @@ __host__ __device__ inline int tg_rule(int emission)
 
 struct GeoArgs {
     const double* params;   // [nb][P]
-    int nb, P, n_spots, n_theta, n_phi, n_phase, n_fp, oblate, emission;
+    int nb, P, n_spots, n_theta, n_phi, n_phase, n_fp, oblate, emission, mesh;
     StarD* stars; SpotD* spots; RowD* rows; int* cells;
     double* lookup;         // [rows][2][kNCheb]: H = psi/alpha, lag
     double* tmpl;           // [rows][4][n_fp+1]
@@ -198,11 +198,36 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     const SpotD sp = A.spots[bs];
     if (threadIdx.x == 0) {
         RowD r;
-        const double e0 = sp.theta_lo + (sp.theta_hi - sp.theta_lo) * (double)j / A.n_theta;
-        const double e1 = sp.theta_lo + (sp.theta_hi - sp.theta_lo) * (double)(j + 1) / A.n_theta;
-        const double th = 0.5 * (e0 + e1);
+        double th;
+        r.npix = A.n_phi; r.phi0 = 0.0; r.dphi = sp.dphi;
+        if (A.mesh == 1) {
+            // HEALPix ring i = j + 1 of N_side = n_phi / 4 (Eq 24-29); pixel area pi / (3 N_side^2)
+            const int nside = A.n_phi / 4, i = j + 1;
+            const bool south = i > 2 * nside;
+            const int in = south ? 4 * nside - i : i;
+            double z;
+            if (in < nside) {                                                      // Eq 24-25
+                z = 1.0 - (double)in * (double)in / (3.0 * (double)nside * (double)nside);
+                r.npix = 4 * in;
+                r.dphi = kPi / (2.0 * (double)in);
+                r.phi0 = r.dphi * 0.5;
+            } else {                                                               // Eq 26-27
+                z = 4.0 / 3.0 - 2.0 * (double)in / (3.0 * (double)nside);
+                r.npix = 4 * nside;
+                r.dphi = kPi / (2.0 * (double)nside);
+                r.phi0 = r.dphi * (1.0 - 0.5 * (double)((in - nside + 1) % 2));
+            }
+            th = acos(south ? -z : z);                                             // Eq 28
+            r.dOmega = kPi / (3.0 * (double)nside * (double)nside);
+            r.dcos = r.dOmega / r.dphi;
+        } else {
+            const double e0 = sp.theta_lo + (sp.theta_hi - sp.theta_lo) * (double)j / A.n_theta;
+            const double e1 = sp.theta_lo + (sp.theta_hi - sp.theta_lo) * (double)(j + 1) / A.n_theta;
+            th = 0.5 * (e0 + e1);
+            r.dcos = cos(e0) - cos(e1);
+            r.dOmega = r.dcos * sp.dphi;
+        }
         r.theta = th;
-        r.dcos = cos(e0) - cos(e1);
         const double ct = cos(th), sth = sin(th);
         const double R = st.Re * (1.0 + st.o2 * ct * ct);                         // Eq 7
         const double u = st.Rs / R;
@@ -223,14 +248,13 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         }
         r.log10g = log10(st.g0 * gr);
         r.c_dt = st.Re - R + st.Rs * log((st.Re - st.Rs) / (R - st.Rs));           // Eq 16
-        r.dOmega = r.dcos * sp.dphi;
         r.alpha_max = 0.5 * kPi + fabs(atan(f));                                   // visible rays: alpha <= pi/2 + |eta|
         r.psi_max = 0.0;
         r.bg = 0; r.wg[0] = r.wg[1] = r.wg[2] = r.wg[3] = 0.0;
         if (A.emission != PPM_EMISSION_BLACKBODY && !st.status)
             axis_w4(A.axg, A.ng, r.log10g, tg_rule(A.emission),
                     r.bg, r.wg);
-        r.n_active = 0; r.visible = 0; r.pad = 0;
+        r.n_active = 0; r.visible = 0;
         row = r;
         base_s = 0;
     }
@@ -241,8 +265,9 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     for (int m0 = 0; m0 < A.n_phi; m0 += blockDim.x) {
         const int m = m0 + threadIdx.x;
         bool act = false;
-        if (m < A.n_phi && !st.status) {
-            const double dphi_m = __dadd_rn(-sp.W, __dmul_rn((double)m + 0.5, sp.dphi));
+        if (m < row.npix && !st.status) {
+            const double dphi_m = (A.mesh == 1) ? __dadd_rn(__dadd_rn(row.phi0, __dmul_rn((double)m, row.dphi)), -sp.phi_c)
+                                                : __dadd_rn(-sp.W, __dmul_rn((double)m + 0.5, sp.dphi));
             const double cd = __dadd_rn(__dmul_rn(ct, sp.cos_tc), __dmul_rn(__dmul_rn(sth, sp.sin_tc), cos(dphi_m)));
             act = (cd >= sp.cos_z);
             if (act && sp.zeta_m > 0.0) {

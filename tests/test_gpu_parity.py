@@ -271,3 +271,26 @@ def test_terms_that_underflow_take_the_guarded_loop():
     assert big.any() and (~big).any()
     assert np.max(np.abs(g[big] - ref[big]) / ref[big]) <= TOL
     assert np.all(g[~big] <= 1e-240)
+
+
+@pytest.mark.parametrize("emission,precision", [(0, 0), (2, 0), (2, 1)])
+def test_healpix_mesh(emission, precision):
+    """mesh = 1: the paper's HEALPix ring mesh over the whole surface (Eq 24-29), two spots (cap + ring with an omitted
+    cap) selected by the centre-in mask; masks bit-exact, flux at the path's tolerance."""
+    nside = 24
+    conf = gen.config_c3(n_cells=8, n_phase=21, n_energy=40)
+    conf["cfg"] = dict(conf["cfg"], n_theta=4 * nside - 1, n_phi=4 * nside, mesh=1, emission=emission)
+    if emission == 0:
+        conf["params"] = conf["params"].copy()
+        conf["params"][0, [8 + 3, 16 + 3]] = 6.4
+    g, st, ctx = gpu_flux(conf, precision=precision)
+    ref, so = oracle_flux(conf)
+    assert st[0] == 0 and so == 0 and ref.max() > 0
+    assert max_rel_err(g[0], ref) <= (TOL32 if precision else TOL)
+    mask = ctx.debug_mask()
+    nt = 4 * nside - 1
+    for s in range(2):
+        sp = o.spot(*conf["params"][0, 8 + 8 * s: 8 + 8 * s + 7])
+        assert np.array_equal(mask[s * nt:(s + 1) * nt], o.spot_mask_healpix(sp, nside))
+    rows = ctx.debug_rows()
+    assert np.allclose(rows[:nt, 11], np.pi / (3 * nside ** 2), rtol=1e-15)      # equal-area pixels (PAPER.md:306)
