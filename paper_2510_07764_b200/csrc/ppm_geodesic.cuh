@@ -27,7 +27,10 @@ __device__ inline void geo_integrals(double u, double sa, double cabs, int g, do
 {
     const double k = u / (1.0 - u), sa2 = sa * sa, ca2 = cabs * cabs;
     const double q0 = (2.0 - k) * sa2;
-    const double layer = (q0 > 0.0) ? cabs / sqrt(q0) : 1.0;
+    // width of the layer at x = 0 where D turns from cos^2(alpha) into x^2 q.  At the periastron call (cos(alpha) = 0
+    // exactly) there is no layer: x / sqrt(D) = 1 / sqrt(q) is smooth on [0, 1] (nearest zero of q at |x| >= 0.6 i for
+    // u <= 0.56) and four dyadic panels resolve it to round-off.
+    const double layer = (cabs == 0.0) ? 0.0625 : ((q0 > 0.0) ? cabs / sqrt(q0) : 1.0);
     const double gx = c_glx[g], gw = c_glw[g];
     double s1 = 0.0, s2 = 0.0;
     double hi = 1.0;
@@ -312,10 +315,11 @@ __global__ void __launch_bounds__(kNCheb * kNGL) k_lookup(GeoArgs A)
     double psi, lag;
     geo_psi_lag(r.u, alpha, g, psi, lag);
     if (g == 0) { fH[j] = psi / alpha; fG[j] = lag; }
-    if (threadIdx.x < 32) {                                      // warp 0: psi at the largest visible emission angle
+    if (threadIdx.x >= kNCheb * kNGL - 32) {                     // last warp (its own nodes, alpha -> 0, are the cheapest):
+                                                                 // psi at the largest visible emission angle
         double pm, lm;
         geo_psi_lag(r.u, r.alpha_max, g, pm, lm);
-        if (threadIdx.x == 0) A.rows[rid].psi_max = pm;
+        if (threadIdx.x == kNCheb * kNGL - 32) A.rows[rid].psi_max = pm;
     }
     if (threadIdx.x < 4 * kNCheb) ctab[threadIdx.x] = cospi((double)threadIdx.x / (2.0 * kNCheb));   // cos(pi m / 128), m < 256
     __syncthreads();
