@@ -666,13 +666,18 @@ double orc_interp4(const orc_atm* A, int strategy, double logT, double logg, dou
 
 /* I(E', mu): emission 0 = isotropic blackbody Eq C.5; 1,2 = table,
  * I = T^3 10^v (reading R13a).  E' in keV, returns keV^0 s^-1 cm^-2 sr^-1 (per keV, times keV). */
+static int g_beaming = 0;   /* blackbody beaming law: 0 isotropic; 1 prop. to cos^2(sigma'); 2 prop. to sin^2(sigma')
+                             * ("simple parametric laws"; cos(sigma') = mu, reading R23) */
 static double intensity(int emission, const orc_atm* A, double log10T, double log10g, double Ep, double mu)
 {
     const double kB = ORC_KB_J_K / ORC_E_C / 1.0e3;
     double T = pow(10.0, log10T), kT = kB * T;
     if (emission == 0) {
         double h = ORC_H_J_S / ORC_E_C / 1.0e3, c = ORC_C_M_S * 100.0;
-        return 2.0 / (h * h * h * c * c) * Ep * Ep * Ep / expm1(Ep / kT);
+        double I = 2.0 / (h * h * h * c * c) * Ep * Ep * Ep / expm1(Ep / kT);
+        if (g_beaming == 1) I *= mu * mu;
+        else if (g_beaming == 2) I *= 1.0 - mu * mu;
+        return I;
     }
     double v = orc_interp4(A, emission, log10T, log10g, mu, log10(Ep / kT));
     return T * T * T * pow(10.0, v);
@@ -694,6 +699,7 @@ typedef struct {
     int32_t n_spots, n_theta, n_phi, n_phase, n_fp, n_energy, emission, oblate;
     int32_t mesh;    /* 0: per-spot theta x phi bounding-box grid (reading R1); 1: HEALPix rings (Eq 24-29) with
                         N_side = n_phi / 4, n_theta = 4 N_side - 1, the same mesh for every spot */
+    int32_t beaming; /* emission 0 only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma') */
 } orc_config;
 
 #define ORC_U_MAX 0.560     /* supported compactness domain (reading R4) */
@@ -727,6 +733,7 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
     orc_star star; orc_star_init(params[0], params[1], params[2], cfg->oblate, &star);
     int status = check_domain(cfg, params, &star);
     if (status) { for (size_t i = 0; i < (size_t)nk * nE; ++i) flux[i] = NAN; return status; }
+    g_beaming = cfg->emission == 0 ? cfg->beaming : 0;   /* set before the parallel region; one evaluation at a time */
     const double cosi = params[3], D_cm = params[4] * 1.0e3 * ORC_PC_M * 100.0, phi_off = params[6];
     const double kB = ORC_KB_J_K / ORC_E_C / 1.0e3;
     (void)kB;

@@ -45,7 +45,7 @@ class _Atm(C.Structure):
 class _Config(C.Structure):
     _fields_ = [("n_spots", C.c_int32), ("n_theta", C.c_int32), ("n_phi", C.c_int32), ("n_phase", C.c_int32),
                 ("n_fp", C.c_int32), ("n_energy", C.c_int32), ("emission", C.c_int32), ("oblate", C.c_int32),
-                ("mesh", C.c_int32)]
+                ("mesh", C.c_int32), ("beaming", C.c_int32)]
 
 
 def _sig(name, res, args):
@@ -249,7 +249,8 @@ def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=Fals
     energies = _f64(energies)
     params = _f64(params)
     c = _Config(cfg["n_spots"], cfg["n_theta"], cfg["n_phi"], cfg["n_phase"], cfg["n_fp"],
-                len(energies), cfg["emission"], int(cfg.get("oblate", 1)), int(cfg.get("mesh", 0)))
+                len(energies), cfg["emission"], int(cfg.get("oblate", 1)), int(cfg.get("mesh", 0)),
+                int(cfg.get("beaming", 0)))
     assert params.shape == (8 + 8 * cfg["n_spots"],)
     if cfg["emission"] != 0:
         assert atm is not None

@@ -296,3 +296,25 @@ def test_p16_loglike_is_poisson_logpmf():
     assert abs(-2 * (ll_m - ll_d) / chi2 - 1.0) < 0.02
     # Eq 56-57 helper
     assert abs(o.chi2(m_big, d_big) - 1e6 / m_big.sum() * chi2) < 1e-9 * chi2
+
+
+# ---------------------------------------------------------------------------------------- beaming laws
+def test_beaming_laws_closed_form_and_linearity(golden):
+    """Blackbody with the parametric beaming laws prop. to cos^2(sigma'), sin^2(sigma') (reading R23).
+    Face-on cap of pin P10 (non-rotating sphere, sigma' = alpha): integrating Eq 21 over the cap gives
+      F_cos2 / F_iso = (1 + cos^2 a_z) / 2,   F_sin2 / F_iso = sin^2(a_z) / 2,
+    with a_z the emission angle at the cap's rim; and for ANY geometry F_iso = F_cos2 + F_sin2 (the laws add to 1)."""
+    pins = {(q, float(E)): float(v) for q, E, v in golden("cap_flux_pins.txt")}
+    a_z = pins[("alpha_zeta", 0.0)]
+    p = gen.pack_params(1.4, 12.0, 0.0, 1.0, 0.2, spots=[(0.0, 0.0, 0.2, LT)])
+    f = {}
+    for b in (0, 1, 2):
+        cfg = dict(_bb_cfg(n_cells=256, n_phase=2, n_fp=8, oblate=0), beaming=b)
+        f[b] = _run(cfg, p)[0]
+    assert np.max(np.abs(f[1] / f[0] / ((1 + np.cos(a_z) ** 2) / 2) - 1)) < 2e-5
+    assert np.max(np.abs(f[2] / f[0] / (np.sin(a_z) ** 2 / 2) - 1)) < 2e-3          # rim-weighted: mask edge error
+    # linearity on a rotating oblate geometry
+    p2 = gen.pack_params(1.4, 12.0, 400.0, np.cos(1.1), 0.2, spots=[(0.8, 0.3, 0.6, LT)])
+    g = {b: _run(dict(_bb_cfg(n_cells=24, n_phase=16, oblate=1), beaming=b), p2) for b in (0, 1, 2)}
+    assert np.max(np.abs((g[1] + g[2]) / g[0] - 1)) < 1e-13
+    assert np.all(g[1] >= 0) and np.all(g[2] >= 0) and g[2].max() > 0
