@@ -76,6 +76,8 @@ typedef struct {
     int32_t mesh;       /* 0: per-spot colatitude x azimuth bounding-box grid (reading R1);
                            1: HEALPix ring scheme over the whole surface (Eq 24-29), the same mesh
                               for every spot: n_phi = 4 N_side, n_theta = 4 N_side - 1 rings, pixel area pi/(3 N_side^2) */
+    int32_t beaming;    /* blackbody emission only: 0 isotropic, 1 I prop. to cos^2(sigma'),
+                           2 I prop. to sin^2(sigma'), cos(sigma') = mu = delta cos(sigma) (Eq 20) */
 } ppm_config;
 
 /* Create a context: copies the energy grid (host, [n_energy], keV, strictly increasing),

@@ -22,7 +22,7 @@ class PPMError(RuntimeError):
 
 class _Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_spots", "n_theta", "n_phi", "n_phase", "n_fp", "n_energy", "emission",
-                                         "precision", "oblate", "max_batch", "device", "mesh")]
+                                         "precision", "oblate", "max_batch", "device", "mesh", "beaming")]
 
 
 # every symbol include/ppm.h declares: name -> (restype, argtypes)
@@ -120,7 +120,7 @@ class PPM:
                                                                 ("n_spots", "n_theta", "n_phi", "n_phase"))
         c = _Config(self.n_spots, self.n_theta, self.n_phi, self.n_phase, int(cfg.get("n_fp", 0)), self.n_energy,
                     int(cfg["emission"]), int(precision), int(cfg.get("oblate", 1)), int(max_batch), int(device),
-                    int(cfg.get("mesh", 0)))
+                    int(cfg.get("mesh", 0)), int(cfg.get("beaming", 0)))
         self.P = 8 + 8 * self.n_spots
         self.max_batch = int(max_batch)
         with torch.cuda.device(self.device):

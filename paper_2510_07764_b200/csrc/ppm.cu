@@ -211,6 +211,8 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
     ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
     ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
+    ARG(cfg->beaming >= 0 && cfg->beaming <= 2, "beaming must be 0, 1 or 2");
+    ARG(cfg->beaming == 0 || cfg->emission == PPM_EMISSION_BLACKBODY, "beaming laws apply to blackbody emission only");
     ARG(cfg->mesh == 0 || cfg->mesh == 1, "mesh must be 0 (theta x phi box per spot) or 1 (HEALPix rings)");
     ARG(cfg->mesh == 0 || (cfg->n_phi % 4 == 0 && cfg->n_theta == cfg->n_phi - 1),
         "HEALPix mesh: n_phi = 4 N_side and n_theta = 4 N_side - 1");
@@ -480,7 +482,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.nmu = table ? c->nmu : 0; A.nx = table ? c->nx : 0;
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
-    A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh;
+    A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh; A.beaming = g.beaming;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     dim3 grid(c->nchunk, c->npg, nb * c->n_etile);

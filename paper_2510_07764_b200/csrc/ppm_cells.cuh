@@ -22,6 +22,7 @@ struct CellArgs {
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
     int nchunk, rows_per_chunk, nw, n_etile, mesh;
+    int beaming;             // blackbody only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma')
 };
 
 // ---- K4: collapse the 4-D table to the row's (mu x logx) slice: T is per spot, g per row -------
@@ -123,6 +124,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
         const double* F = T;
         const double* Z = T + n1;
         const double* PO = T + 2 * n1;
+        const double* MU = T + 3 * n1;
         const int* cl = A.cells + (size_t)rid * A.n_phi;
         const double po0 = PO[0];
         for (int base = 0; base < nact; base += 32) {
@@ -144,6 +146,10 @@ __global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
                 if (Fp != 0.0) {
                     pa = zp / sp.kT;
                     pb = Fp * (2.0 / (kH_keV_s * kH_keV_s * kH_keV_s * kC_cm_s * kC_cm_s)) * zp * zp * zp;
+                    if (A.beaming) {                                            // cos(sigma') = mu_p (Eq 20)
+                        const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+                        pb *= (A.beaming == 1) ? mup * mup : 1.0 - mup * mup;
+                    }
                 }
             }
             unsigned todo = __ballot_sync(0xffffffffu, Fp != 0.0);

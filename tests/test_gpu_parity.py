@@ -294,3 +294,17 @@ def test_healpix_mesh(emission, precision):
         assert np.array_equal(mask[s * nt:(s + 1) * nt], o.spot_mask_healpix(sp, nside))
     rows = ctx.debug_rows()
     assert np.allclose(rows[:nt, 11], np.pi / (3 * nside ** 2), rtol=1e-15)      # equal-area pixels
+
+
+@pytest.mark.parametrize("beaming", [1, 2])
+def test_blackbody_beaming_laws(beaming):
+    """cos^2 / sin^2 beaming on the OS1-like set-up: M = 1.4, R = 12 km, D = 200 pc, kT = 0.35 keV,
+    monochromatic 1 keV, extended spot zeta = 1 rad, oblate star at 400 Hz."""
+    E = np.array([1.0])
+    cfg = dict(n_spots=1, n_theta=40, n_phi=40, n_phase=32, n_fp=192, emission=0, oblate=1, beaming=beaming)
+    p = gen.pack_params(1.4, 12.0, 400.0, np.cos(np.deg2rad(70.0)), 0.2,
+                        spots=[(np.deg2rad(50.0), 0.0, 1.0, gen.log10T_of_kT(0.35))])
+    conf = dict(cfg=cfg, energies=E, params=p[None, :])
+    g, st, _ = gpu_flux(conf)
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and ref.max() > 0 and max_rel_err(g[0], ref) <= TOL
