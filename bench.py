@@ -43,11 +43,10 @@ FLOP_PER_TRIPLE = 86.0          # SURVEY.md 8(d) accounting constant (FMA = 2 fl
 # nominal FP64 vector peak: 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_cells_tab launch, from the one `ncu --set full` capture of each
-# workload that has one (profiles/r1c_k_cells_tab_T_full.md); other workloads report null
-NCU_TRAFFIC_BYTES = {"T": 71.835392e6 + 53.226752e6}
-# FP64 instructions the kernel executes per triple: 16.43 DFMA + 7.11 DADD + 1.42 DMUL in that capture, less the two
-# DFMA of the exp2 polynomial's degree 10 -> 8 change made after it
-EXECUTED_FLOP_PER_TRIPLE = 2 * 14.43 + 7.11 + 1.42
+# workload that has one (profiles/r1d_k_cells_tab_T_full.md); other workloads report null
+NCU_TRAFFIC_BYTES = {"T": 74.063104e6 + 54.766336e6}
+# FP64 instructions the kernel executes per triple in that capture: 14.30 DFMA + 7.11 DADD + 1.42 DMUL
+EXECUTED_FLOP_PER_TRIPLE = 2 * 14.30 + 7.11 + 1.42
 METRIC = "pulse-profile evaluations per second"
 UNIT = "evals/s"
 

@@ -233,7 +233,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     c->n_fp = cfg->n_fp > 0 ? cfg->n_fp : std::max(192, 2 * cfg->n_phase);           // reading R2
     c->h_en.assign(energies, energies + cfg->n_energy);
     // launch geometry of the cell kernel
-    // 16 warps x 128 registers fill the register file; 32 warps x 64 registers measured slower (profiles/r1c_variants.md)
+    // 16 warps x 128 registers fill the register file; 32 warps x 64 registers measured slower (profiles/r1d_k_cells_tab_T_full.md)
     c->nw = std::min(16, cfg->n_phase);
     c->npg = (cfg->n_phase + c->nw - 1) / c->nw;
     const int need = (cfg->n_energy + 31) / 32;
