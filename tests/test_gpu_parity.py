@@ -332,3 +332,18 @@ def test_bench_line_contract():
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] == 2 * 16 * 8 and e["d2h_bytes_per_step"] == 2 * 12
+
+
+def test_random_prior_vectors_sweep():
+    """48 seeded vectors from C5's priors (M 1-3, R 8-16 km, 200-700 Hz, any inclination, spot radii up to 1 rad) at
+    reduced grid size, every bin against the oracle: FP64 path at 1e-9, FP32-interpolation path at 1e-4."""
+    import torch
+    conf = gen.config_c5(n_vec=48, n_cells=16, n_phase=20, n_energy=40, seed=gen.SEED0 + 77)
+    refs = [oracle_flux(conf, b) for b in range(48)]
+    for precision, tol in ((0, TOL), (1, TOL32)):
+        ctx = make_ctx(conf, precision=precision)
+        flux, status = ctx.evaluate(torch.as_tensor(conf["params"], device="cuda"))
+        g, st = flux.cpu().numpy(), status.cpu().numpy()
+        for b, (ref, so) in enumerate(refs):
+            assert st[b] == so == 0
+            assert max_rel_err(g[b], ref) <= tol, (precision, b)
