@@ -726,8 +726,11 @@ static int check_domain(const orc_config* cfg, const double* p, const orc_star* 
     return status;
 }
 
-int orc_evaluate(const orc_config* cfg, const double* energies, const double* params, const orc_atm* atm,
-                 const int32_t* phase_sel, int n_phase_sel, double* flux, double* margin_out)
+/* tmap (optional): per-cell effective temperature map log10 T[n_spots][n_theta][n_phi] ("a full
+ * surface temperature map T_eff(theta, phi)"); a cell of the mesh emits iff it passes the spot's geometric mask AND
+ * its map entry is finite (NaN = not emitting); the spot's own log10 T parameter is then ignored (reading R24). */
+static int evaluate_impl(const orc_config* cfg, const double* energies, const double* params, const orc_atm* atm,
+                         const double* tmap, const int32_t* phase_sel, int n_phase_sel, double* flux, double* margin_out)
 {
     const int nk = phase_sel ? n_phase_sel : cfg->n_phase, nE = cfg->n_energy, nfp = cfg->n_fp;
     orc_star star; orc_star_init(params[0], params[1], params[2], cfg->oblate, &star);
@@ -768,8 +771,10 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
             }
 #define CELL_DPHI(m) (cfg->mesh == 1 ? (hp_phi0 + (double)(m) * hp_dphi) - sp.phi_c : cell_dphi(&bx, (m)))
             /* active azimuths of this ring */
+            const double* trow = tmap ? tmap + ((size_t)sidx * cfg->n_theta + j) * cfg->n_phi : NULL;
+#define CELL_ON(m) (cell_active(&sp, row.theta, CELL_DPHI(m)) && (!trow || isfinite(trow[(m)])))
             int n_act = 0;
-            for (int m = 0; m < npix; ++m) n_act += cell_active(&sp, row.theta, CELL_DPHI(m));
+            for (int m = 0; m < npix; ++m) n_act += CELL_ON(m);
             if (n_act == 0) continue;
             double mg;
             int visible = orc_template(&star, &row, cosi, D_cm, dOmega, nfp, F, z, po, mu, NULL, &mg, NULL, NULL);
@@ -778,7 +783,8 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
             /* O5 shift-and-add */
             for (int m = 0; m < npix; ++m) {
                 double dphi_m = CELL_DPHI(m);
-                if (!cell_active(&sp, row.theta, dphi_m)) continue;
+                if (!CELL_ON(m)) continue;
+                const double cell_log10T = trow ? trow[m] : sp.log10T;
                 double phi_m = sp.phi_c + dphi_m;
                 for (int kk = 0; kk < nk; ++kk) {
                     int k = phase_sel ? phase_sel[kk] : kk;
@@ -794,7 +800,7 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
                     if (Fp == 0.0) continue;
                     for (int e = 0; e < nE; ++e) {
                         double E = energies[e];
-                        double I = intensity(cfg->emission, atm, sp.log10T, row.log10g, zp * E, mup);
+                        double I = intensity(cfg->emission, atm, cell_log10T, row.log10g, zp * E, mup);
                         acc[(size_t)kk * nE + e] += Fp * I / E;                               /* Eq 47 */
                     }
                 }
@@ -809,6 +815,18 @@ int orc_evaluate(const orc_config* cfg, const double* energies, const double* pa
     }
     if (margin_out) *margin_out = margin_all;
     return 0;
+}
+
+int orc_evaluate(const orc_config* cfg, const double* energies, const double* params, const orc_atm* atm,
+                 const int32_t* phase_sel, int n_phase_sel, double* flux, double* margin_out)
+{
+    return evaluate_impl(cfg, energies, params, atm, NULL, phase_sel, n_phase_sel, flux, margin_out);
+}
+
+int orc_evaluate_map(const orc_config* cfg, const double* energies, const double* params, const orc_atm* atm,
+                     const double* tmap, const int32_t* phase_sel, int n_phase_sel, double* flux, double* margin_out)
+{
+    return evaluate_impl(cfg, energies, params, atm, tmap, phase_sel, n_phase_sel, flux, margin_out);
 }
 
 /* ------------------------------------------------------------------------------------

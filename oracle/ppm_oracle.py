@@ -77,6 +77,8 @@ _interp4 = _sig("orc_interp4", C.c_double, [C.POINTER(_Atm), C.c_int] + [C.c_dou
 _intensity = _sig("orc_intensity", C.c_double, [C.c_int, C.POINTER(_Atm)] + [C.c_double] * 4)
 _evaluate = _sig("orc_evaluate", C.c_int,
                  [C.POINTER(_Config), _dp, _dp, C.POINTER(_Atm), _ip, C.c_int, _dp, _dp])
+_evaluate_map = _sig("orc_evaluate_map", C.c_int,
+                     [C.POINTER(_Config), _dp, _dp, C.POINTER(_Atm), _dp, _ip, C.c_int, _dp, _dp])
 _fold = _sig("orc_fold", None, [_dp, C.c_int, C.c_int, C.c_int, C.c_int, _ip, _dp, _dp, C.c_double, _dp])
 _loglike = _sig("orc_loglike", C.c_double, [_dp, _dp, _dp, C.c_int, C.c_int, C.c_double])
 _hp_ring = _sig("orc_healpix_ring", None, [C.c_int, C.c_int, _dp, C.POINTER(C.c_int), _dp, _dp])
@@ -243,7 +245,7 @@ def intensity(emission, atm, log10T, log10g, Ep, mu):
 
 
 # ---- evaluation ------------------------------------------------------------------------
-def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=False):
+def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=False, tmap=None):
     """cfg: dict(n_spots,n_theta,n_phi,n_phase,n_fp,n_energy?,emission,oblate).  params: 1-D vector.
     Returns (flux[n_k][n_energy], status[, margin])."""
     energies = _f64(energies)
@@ -261,8 +263,13 @@ def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=Fals
         nk, selp = cfg["n_phase"], None
     flux = np.zeros((nk, len(energies)))
     mg = C.c_double()
-    status = _evaluate(C.byref(c), _p(energies), _p(params), C.byref(atm.c) if atm is not None else None,
-                       selp, nk, _p(flux), C.byref(mg))
+    ap = C.byref(atm.c) if atm is not None else None
+    if tmap is not None:                       # per-cell log10 T map [n_spots][n_theta][n_phi], NaN = not emitting
+        tmap = _f64(tmap)
+        assert tmap.shape == (cfg["n_spots"], cfg["n_theta"], cfg["n_phi"])
+        status = _evaluate_map(C.byref(c), _p(energies), _p(params), ap, _p(tmap), selp, nk, _p(flux), C.byref(mg))
+    else:
+        status = _evaluate(C.byref(c), _p(energies), _p(params), ap, selp, nk, _p(flux), C.byref(mg))
     if return_margin:
         return flux, status, mg.value
     return flux, status
