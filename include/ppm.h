@@ -107,6 +107,14 @@ int ppm_set_response(ppm_ctx* ctx, int n_channel, int band_w, const int32_t* fir
  * (Eq 21); status_dev [B] (may be NULL). */
 int ppm_evaluate(ppm_ctx* ctx, const double* params_dev, int B, double* flux_dev, int32_t* status_dev);
 
+/* S0-S5 with a per-cell effective-temperature map ("a full surface temperature map T_eff(theta,
+ * phi)"; reading R24): logT_map_dev [B][n_spots][n_theta][n_phi] holds log10 T_eff/K of every cell of every spot's mesh
+ * (box grid or HEALPix); a cell emits iff it passes the spot's geometric mask (centre within zeta, outside the omitted
+ * cap) AND its entry is finite -- NaN marks a cell that does not emit.  The spots' own log10 T parameters are ignored.
+ * Needs emission = PPM_EMISSION_TABLE_MIXED (linear in log T) and precision = 0; otherwise PPM_ERR_STATE. */
+int ppm_evaluate_map(ppm_ctx* ctx, const double* params_dev, const double* logT_map_dev, int B, double* flux_dev,
+                     int32_t* status_dev);
+
 /* S6: C[b][k][c] = sum_e F_t[b][k][e] exp(-N_H20[b] tau_ref[e]) RSP0[e][c]  (Eq 22-23, 55).
  * N_H20 is params[b][5].  counts_dev [B][n_phase][n_channel], counts/s. */
 int ppm_fold_response(ppm_ctx* ctx, const double* flux_dev, const double* params_dev, int B,

@@ -32,6 +32,7 @@ EXPORTS = {
     "ppm_load_atmosphere": (C.c_int, [_vp, _dp, C.c_int, _dp, C.c_int, _dp, C.c_int, _dp, C.c_int, _vp, C.c_int]),
     "ppm_set_response": (C.c_int, [_vp, C.c_int, C.c_int, _ip, _vp, C.c_int, _dp]),
     "ppm_evaluate": (C.c_int, [_vp, _vp, C.c_int, _vp, _vp]),
+    "ppm_evaluate_map": (C.c_int, [_vp, _vp, _vp, C.c_int, _vp, _vp]),
     "ppm_fold_response": (C.c_int, [_vp, _vp, _vp, C.c_int, _vp]),
     "ppm_loglike": (C.c_int, [_vp, _vp, C.c_int, _vp, _vp, C.c_double, _vp]),
     "ppm_evaluate_host": (C.c_int, [_vp, _dp, C.c_int, _dp, _ip]),
@@ -174,6 +175,20 @@ class PPM:
             status = t.empty((B,), dtype=t.int32, device=self.device)
         _check(self.lib.ppm_evaluate(self._h, _dev(params, t.float64, "params"), B, _dev(flux, t.float64, "flux"),
                                      _dev(status, t.int32, "status")))
+        return flux, status
+
+    def evaluate_map(self, params, logT_map, flux=None, status=None):
+        """ppm_evaluate_map: logT_map [B][n_spots][n_theta][n_phi] float64 CUDA tensor, NaN = cell does not emit."""
+        t = self.torch
+        B = params.shape[0]
+        if tuple(logT_map.shape) != (B, self.n_spots, self.n_theta, self.n_phi):
+            raise PPMError("logT_map must have shape [B][n_spots][n_theta][n_phi]")
+        if flux is None:
+            flux = t.empty((B, self.n_phase, self.n_energy), dtype=t.float64, device=self.device)
+        if status is None:
+            status = t.empty((B,), dtype=t.int32, device=self.device)
+        _check(self.lib.ppm_evaluate_map(self._h, _dev(params, t.float64, "params"), _dev(logT_map, t.float64, "logT_map"),
+                                         B, _dev(flux, t.float64, "flux"), _dev(status, t.int32, "status")))
         return flux, status
 
     def fold_response(self, flux, params, counts=None):

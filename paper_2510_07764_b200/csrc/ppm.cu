@@ -18,6 +18,7 @@
 #include "ppm_geodesic.cuh"
 #include "ppm_cells.cuh"
 #include "ppm_cells32.cuh"
+#include "ppm_cells_map.cuh"
 #include "ppm_observe.cuh"
 
 using namespace ppm;
@@ -436,7 +437,27 @@ static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, 
     }
 }
 
-static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* flux_dev, int32_t* status_dev)
+// shared memory of k_cells_map with `nw` warps (ppm_cells_map.cuh layout)
+static size_t cells_map_smem(const ppm_ctx* c, int nw)
+{
+    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 16) + 2 * (size_t)c->nmu * c->nx +
+                             4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT);
+}
+
+template <int EPL>
+static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    switch (c->npl) {
+    case 1:  return launch_cells(c, k_cells_map<EPL, 1>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_map<EPL, 3>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_map<EPL, 5>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_map<EPL, 7>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_map<EPL, 9>, a, grid, threads, smem);
+    }
+}
+
+static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* flux_dev, int32_t* status_dev,
+                        const double* tmap_dev = nullptr)
 {
     const ppm_config& g = c->cfg;
     const bool table = g.emission != PPM_EMISSION_BLACKBODY;
@@ -446,6 +467,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     G.stars = c->d_stars; G.spots = c->d_spots; G.rows = c->d_rows; G.cells = c->d_cells;
     G.lookup = c->d_lookup; G.tmpl = c->d_tmpl;
     G.axT = c->d_axT; G.nT = c->nT; G.axg = c->d_axg; G.ng = c->ng;
+    G.tmap = tmap_dev;
     const int rows = nb * c->RT;
     prof_begin(c, KID_STAR);
     k_star<<<(nb + 63) / 64, 64, 0, c->stream>>>(G);
@@ -462,7 +484,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     k_template<<<rows, 128, tsm, c->stream>>>(G);
     prof_end(c);
     c->launches += 4;
-    if (table) {
+    if (table && !tmap_dev) {
         SliceArgs S;
         S.spots = c->d_spots; S.rows = c->d_rows; S.values = c->d_values; S.slices = c->d_slices;
         S.n_theta = g.n_theta; S.nT = c->nT; S.ng = c->ng; S.nmu = c->nmu; S.nx = c->nx;
@@ -472,7 +494,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
         prof_end(c);
         c->launches += 1;
     }
-    CellArgs A;
+    CellArgs A{};
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
     A.slices = c->d_slices; A.axmu = c->d_axmu; A.uef = c->d_uef; A.en = c->d_en;
     A.partial = c->d_partial; A.pairs = c->d_pairs;
@@ -485,9 +507,31 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh; A.beaming = g.beaming;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
-    dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
-    prof_begin(c, KID_CELLS);
-    int rc = dispatch_cells(c, table, A, grid, c->nw * 32, smem);
+    int rc;
+    if (tmap_dev) {
+        // temperature-map mode: two FP64 node slices in shared memory -> fewer warps (output phases) per block
+        int nwm = 0;
+        for (int v : {8, 6, 4, 2, 1}) if (cells_map_smem(c, v) <= 227 * 1024) { nwm = v; break; }
+        if (!nwm) { set_err("temperature-map mode: table and template do not fit in shared memory"); return PPM_ERR_ARG; }
+        nwm = std::min(nwm, g.n_phase);
+        A.nw = nwm;
+        A.tmap = tmap_dev; A.values = c->d_values; A.axT = c->d_axT; A.nT = c->nT; A.ng = c->ng;
+        dim3 grid(c->nchunk, (g.n_phase + nwm - 1) / nwm, nb * c->n_etile);
+        const size_t smem_map = cells_map_smem(c, nwm);
+        prof_begin(c, KID_CELLS);
+        switch (c->epl) {
+        case 1:  rc = dispatch_cells_map<1>(c, A, grid, nwm * 32, smem_map); break;
+        case 2:  rc = dispatch_cells_map<2>(c, A, grid, nwm * 32, smem_map); break;
+        case 4:  rc = dispatch_cells_map<4>(c, A, grid, nwm * 32, smem_map); break;
+        case 5:  rc = dispatch_cells_map<5>(c, A, grid, nwm * 32, smem_map); break;
+        case 8:  rc = dispatch_cells_map<8>(c, A, grid, nwm * 32, smem_map); break;
+        default: rc = dispatch_cells_map<10>(c, A, grid, nwm * 32, smem_map); break;
+        }
+    } else {
+        dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
+        prof_begin(c, KID_CELLS);
+        rc = dispatch_cells(c, table, A, grid, c->nw * 32, smem);
+    }
     prof_end(c);
     if (rc) return rc;
     const int n_out = g.n_phase * g.n_energy;
@@ -517,6 +561,31 @@ extern "C" int ppm_evaluate(ppm_ctx* c, const double* params_dev, int B, double*
         const int nb = std::min(c->SB, B - b0);
         int rc = evaluate_sub(c, params_dev + (size_t)b0 * c->P, nb, flux_dev + (size_t)b0 * fstride,
                               status_dev ? status_dev + b0 : nullptr);
+        if (rc) return rc;
+    }
+    return PPM_OK;
+}
+
+extern "C" int ppm_evaluate_map(ppm_ctx* c, const double* params_dev, const double* logT_map_dev, int B, double* flux_dev,
+                                int32_t* status_dev)
+{
+    ARG(c, "null context");
+    ARG(B >= 0, "B must be >= 0");
+    if (B == 0) return PPM_OK;
+    ARG(params_dev && logT_map_dev && flux_dev, "null pointer");
+    if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
+    if (c->cfg.emission != PPM_EMISSION_TABLE_MIXED || c->cfg.precision != 0) {
+        set_err("temperature maps need emission = 2 (linear in log T) and precision = 0"); return PPM_ERR_STATE;
+    }
+    if (!c->have_atm) { set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE; }
+    if (c->nT > 64) { set_err("temperature maps support at most 64 log T nodes"); return PPM_ERR_STATE; }
+    CK(cudaSetDevice(c->cfg.device));
+    const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy;
+    const size_t mstride = (size_t)c->RT * c->cfg.n_phi;
+    for (int b0 = 0; b0 < B; b0 += c->SB) {
+        const int nb = std::min(c->SB, B - b0);
+        int rc = evaluate_sub(c, params_dev + (size_t)b0 * c->P, nb, flux_dev + (size_t)b0 * fstride,
+                              status_dev ? status_dev + b0 : nullptr, logT_map_dev + (size_t)b0 * mstride);
         if (rc) return rc;
     }
     return PPM_OK;

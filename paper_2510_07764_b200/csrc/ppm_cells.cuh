@@ -17,6 +17,10 @@ struct CellArgs {
                              //       (h = logx spacing; units of 2^-52 table intervals)
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
+    const double* tmap;      // temperature-map mode: [rows][n_phi] log10 T per cell
+    const double* values;    // temperature-map mode: the 4-D table [nT][ng][nmu][nx]
+    const double* axT;       // temperature-map mode: log T axis [nT]
+    int nT, ng;
     unsigned long long* pairs;   // counter: (cell, phase) pairs with F_p != 0 (energy tile 0 only)
     double x0_over_h, inv_h;
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;

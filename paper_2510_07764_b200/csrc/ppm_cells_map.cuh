@@ -1,0 +1,247 @@
+// ppm_cells_map.cuh -- S4 + S5 for a per-cell effective-temperature map T_eff(theta, phi) (the paper's
+// "full surface temperature map"; reading R24).  Strategy d only (emission = 2: linear in log T and log g).
+// Product path (sm_100a).
+//
+// With one temperature per spot the 4-D table collapses per row to ONE (mu x logx) slice (k_slice).  With a map every
+// cell has its own log T, so a pair needs the slices of the two log T nodes that bracket its cell:
+//   v = (1 - t) v[iT] + t v[iT+1],   f_node = log2(10) sum_mu w_mu [(1 - t) S_iT + t S_iT+1][mu][c] + log2(F_p T^3).
+// k_rows records, per row, which log T intervals its active cells fall in (RowD::tmask).  The block walks those
+// intervals in ascending order; for interval iT it stages the node slices iT and iT+1 -- blended over the row's two
+// log g nodes on the fly from the L2-resident 4-D table -- into two shared-memory buffers (the upper node of one
+// interval is the lower node of the next: ping-pong, one new slice per step), and processes the row's cells of that
+// interval.  Two FP64 slices take 178 KB, so a block has 8 warps (8 output phases) instead of 16.
+// Everything per pair and per triple is k_cells_tab's scheme (fixed-point logx coordinate, fused shuffle pass to
+// per-interval monomial coefficients, Horner + degree-8 exp2), with T, kT and T^3 taken per cell.
+#pragma once
+#include "ppm_cells.cuh"
+
+namespace ppm {
+
+__device__ __forceinline__ double contract4(const double* __restrict__ sp0, int nx, double v0, double v1, double v2, double v3)
+{
+    return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
+}
+
+template <int EPL, int NPL>
+__global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int chunk = blockIdx.x, pg = blockIdx.y;
+    const int b = blockIdx.z / A.n_etile, et = blockIdx.z % A.n_etile;
+    const int k = pg * A.nw + w;
+    const bool kvalid = k < A.n_phase;
+    const int e0 = et * 32 * EPL;
+    const int n1 = A.n_fp + 1;
+    const int nx = A.nx;
+    const int plane = A.nmu * nx;
+    // shared layout (doubles): per warp { KA [KW], KB [KW], R0 (q, qb), R1 (v0, v1), R2 (v2, v3), R3 (1-t, t) [32] as
+    // double2, RI [32] int } | S0 [nmu][nx] | S1 [nmu][nx] | T [4][n1] | MUAX [nmu] | TAX [nT]
+    constexpr int KW = 32 * NPL;
+    constexpr int WARP_DBL = 4 * KW + 4 * 64 + 16;
+    double* wbase = sm + (size_t)w * WARP_DBL;
+    double2* KA = reinterpret_cast<double2*>(wbase);
+    double2* R0 = KA + 2 * KW;
+    double2* R1 = R0 + 32;
+    double2* R2 = R1 + 32;
+    double2* R3 = R2 + 32;
+    int* RI = reinterpret_cast<int*>(R3 + 32);
+    double* Sb0 = sm + (size_t)A.nw * WARP_DBL;
+    double* Sb1 = Sb0 + plane;
+    double* T = Sb1 + plane;
+    double* MUAX = T + 4 * n1;
+    double* TAX = MUAX + A.nmu;
+
+    long long uef[EPL];
+    double acc[EPL];
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) {
+        const int e = e0 + lane + 32 * i;
+        uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
+        acc[i] = 0.0;
+    }
+    const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
+    const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
+    const long long s_top = ((long long)(nx - 1) << 52) - 1;
+    for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
+    for (int i = threadIdx.x; i < A.nT; i += blockDim.x) TAX[i] = A.axT[i];
+
+    const StarD& st = A.stars[b];
+    const double phi_off = st.phi_off;
+    const double phi_out = (double)k / A.n_phase;                               // reading R3
+    const double log10kB = log10(kKB_keV_K);
+    unsigned npairs = 0;
+
+    for (int ri = 0; ri < A.rows_per_chunk; ++ri) {
+        const int rl = chunk + ri * A.nchunk;
+        if (rl >= A.RT) break;
+        const int rid = b * A.RT + rl;
+        const RowD& row = A.rows[rid];
+        const int nact = row.n_active;
+        if (nact == 0 || !row.visible) continue;
+        const SpotD& sp = A.spots[rid / A.n_theta];
+        __syncthreads();
+        {
+            const double* ts = A.tmpl + (size_t)rid * 4 * n1;
+            for (int i = threadIdx.x; i < 4 * n1; i += blockDim.x) T[i] = ts[i];
+        }
+        const double* F = T;
+        const double* Z = T + n1;
+        const double* PO = T + 2 * n1;
+        const double* MU = T + 3 * n1;
+        const int* cl = A.cells + (size_t)rid * A.n_phi;
+        const double* tcell = A.tmap + (size_t)rid * A.n_phi;
+        int node0 = -1, node1 = -1;                                              // log T node held by slice buffer 0 / 1
+        for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
+            const int it = __ffsll((long long)tm) - 1;                           // log T interval [it, it+1]
+            const int pl = (node1 == it) ? 1 : 0;
+            __syncthreads();                                                     // readers of the previous interval are done
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {                                        // h = 0: lower node -> buffer pl; 1: upper -> 1 - pl
+                const int buf = h ? 1 - pl : pl, node = it + h;
+                if ((buf ? node1 : node0) == node) continue;
+                if (buf) node1 = node; else node0 = node;
+                double* dst = buf ? Sb1 : Sb0;
+                const double* src = A.values + ((size_t)node * A.ng + row.bg) * plane;
+                for (int i = threadIdx.x; i < plane; i += blockDim.x) {
+                    double v = 0.0;
+#pragma unroll
+                    for (int gq = 0; gq < 4; ++gq)
+                        if (row.wg[gq] != 0.0) v = fma(row.wg[gq], __ldg(src + (size_t)gq * plane + i), v);
+                    dst[i] = v;
+                }
+            }
+            __syncthreads();
+            if (!kvalid) continue;
+            const double* Slo = pl ? Sb1 : Sb0;
+            const double* Shi = pl ? Sb0 : Sb1;
+            const double po0 = PO[0];
+            for (int base = 0; base < nact; base += 32) {
+                // ---- step A: lane <-> cell; cells of other log T intervals are skipped in this pass over the row ----
+                const int idx = base + lane;
+                double Fp = 0.0, pb = 0.0, tw = 0.0;
+                long long pq = 0;
+                double ww[4] = {0.0, 0.0, 0.0, 0.0};
+                int info = 0;
+                if (idx < nact) {
+                    const int m = cl[idx];
+                    const double lT = tcell[m];
+                    double tt;
+                    if (axis_linear(TAX, A.nT, lT, tt) == it) {
+                        const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi
+                                                    : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
+                        const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
+                        const double phi_p = (s0 - floor(s0)) + po0;                // Eq 45
+                        int lo = 0, hi = A.n_fp;
+                        while (hi - lo > 1) {
+                            const int mid = (lo + hi) >> 1;
+                            if (PO[mid] <= phi_p) lo = mid; else hi = mid;
+                        }
+                        const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
+                        Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                       // Eq 46, linear (reading R11)
+                        const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
+                        const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+                        if (Fp != 0.0) {
+                            const double up = (log10(zp) - (log10kB + lT)) * A.inv_h - A.x0_over_h;
+                            pq = __double2ll_rn(up * kTwo52);
+                            pb = log2(Fp) + 3.0 * lT * kLog2_10;                    // log2(F_p T^3), T of this cell
+                            tw = tt;
+                            int mb;
+                            axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
+#pragma unroll
+                            for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= kLog2_10;
+                            const long long sa = pq + uef_first, sb2 = pq + uef_last;
+                            const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
+                            const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
+                            const int clamped = (sa < 0) || (sb2 > s_top);
+                            info = (mb * nx) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
+                        }
+                    }
+                }
+                const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);
+                const int cnt = __popc(valid);
+                npairs += cnt;
+                __syncwarp();
+                if (Fp != 0.0) {
+                    const int slot = __popc(valid & ((1u << lane) - 1u));
+                    R0[slot] = make_double2(__longlong_as_double(pq), pb);
+                    R1[slot] = make_double2(ww[0], ww[1]);
+                    R2[slot] = make_double2(ww[2], ww[3]);
+                    R3[slot] = make_double2(1.0 - tw, tw);
+                    RI[slot] = info;
+                }
+                __syncwarp();
+                // ---- step B: walk the valid pairs ----
+                for (int pj = 0; pj < cnt; ++pj) {
+                    const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj], r3 = R3[pj];
+                    const int inf = RI[pj];
+                    const long long q = __double_as_longlong(r0.x);
+                    const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
+                    const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
+                    const int soff = (inf & 0x7FFF) + jlo - 1 + NPL * lane;
+                    const int n0 = jlo - 1 + NPL * lane;
+                    double f[NPL + 3];
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn)
+                        f[1 + jn] = fma(r3.y, contract4(Shi + soff + jn, nx, v0, v1, v2, v3),
+                                        fma(r3.x, contract4(Slo + soff + jn, nx, v0, v1, v2, v3), qb));
+                    f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
+                    if (NPL == 1) {
+                        f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
+                        f[3] = __shfl_down_sync(0xffffffffu, f[1], 2);
+                    } else {
+                        f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
+                        f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
+                    }
+                    double2 ka[NPL], kb[NPL];
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn)
+                        cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
+                    if (jlo == 0 || jhi == nx - 2) {      // strategy d: linear in the first / last interval of the axis
+#pragma unroll
+                        for (int jn = 0; jn < NPL; ++jn) {
+                            const int c = n0 + jn;
+                            if (c != 0 && c != nx - 2) continue;
+                            ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
+                            kb[jn] = make_double2(0.0, 0.0);
+                        }
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn) {
+                        KA[NPL * lane + jn] = ka[jn];
+                        KA[NPL * lane + jn + KW] = kb[jn];
+                    }
+                    __syncwarp();
+                    const double2* KAq = KA + (1 - jlo);
+                    const bool clampc = inf & 0x8000;
+#pragma unroll
+                    for (int i = 0; i < EPL; ++i) {
+                        long long s = q + uef[i];
+                        if (clampc) s = s < 0 ? 0 : (s > s_top ? s_top : s);     // reading R13b
+                        const int shi = (int)(s >> 32);
+                        const double2* kp = KAq + (shi >> 20);
+                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                        const double2 c01 = kp[0], c23 = kp[KW];
+                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+                        const double r = y + kMagic;
+                        const int n = __double2loint(r);
+                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
+                        if (n >= -1000) acc[i] += val;
+                    }
+                }
+            }
+        }
+    }
+    if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
+    if (kvalid) {
+        double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) {
+            const int e = e0 + lane + 32 * i;
+            if (e < A.nE) out[e] = acc[i] / A.en[e];                            // the 1/E_e of Eq 47
+        }
+    }
+}
+
+}  // namespace ppm

@@ -48,6 +48,7 @@ struct RowD {
     double wg[4];                                 // log g axis stencil
     int bg, n_active, visible, npix;              // npix: azimuth cells of this row (HEALPix rings differ)
     double phi0, dphi;                            // azimuth of cell m: phi0 + m dphi (HEALPix mesh only)
+    unsigned long long tmask;                     // temperature-map mode: bit i set iff an active cell lies in log T interval i
 };
 
 __host__ __device__ inline int imin_(int a, int b) { return a < b ? a : b; }
@@ -90,6 +91,21 @@ __device__ inline void axis_w4(const double* __restrict__ ax, int n, double x, i
     w[1] = (d0 * d2 * d3) / ((x1 - x0) * (x1 - x2) * (x1 - x3));
     w[2] = (d0 * d1 * d3) / ((x2 - x0) * (x2 - x1) * (x2 - x3));
     w[3] = (d0 * d1 * d2) / ((x3 - x0) * (x3 - x1) * (x3 - x2));
+}
+
+// Linear rule on one axis (the log T axis of a temperature map): x clamped to the axis (reading R13b), interval i with
+// ax[i] <= x <= ax[i+1], t = (x - ax[i]) / (ax[i+1] - ax[i]) -- the arithmetic of axis_w4's AX_LINEAR branch.
+__device__ inline int axis_linear(const double* __restrict__ ax, int n, double x, double& t)
+{
+    x = fmin(fmax(x, ax[0]), ax[n - 1]);
+    int lo = 0, hi = n - 1;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (ax[mid] <= x) lo = mid; else hi = mid;
+    }
+    const int i = imin_(lo, n - 2);
+    t = (x - ax[i]) / (ax[i + 1] - ax[i]);
+    return i;
 }
 
 }  // namespace ppm

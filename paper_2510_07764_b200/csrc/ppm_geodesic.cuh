@@ -118,6 +118,7 @@ struct GeoArgs {
     double* lookup;         // [rows][2][kNCheb]: H = psi/alpha, lag
     double* tmpl;           // [rows][4][n_fp+1]
     const double* axT; int nT; const double* axg; int ng;
+    const double* tmap;     // [rows][n_phi] log10 T per cell, NaN = not emitting (temperature-map mode), or nullptr
 };
 
 __global__ void k_star(GeoArgs A)
@@ -195,6 +196,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     __shared__ RowD row;
     __shared__ int warp_cnt[4];
     __shared__ int base_s;
+    __shared__ unsigned long long tmask_s;
     const int rid = blockIdx.x;                          // (b * n_spots + s) * n_theta + j
     const int j = rid % A.n_theta, bs = rid / A.n_theta, b = bs / A.n_spots;
     const StarD st = A.stars[b];
@@ -257,9 +259,10 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         if (A.emission != PPM_EMISSION_BLACKBODY && !st.status)
             axis_w4(A.axg, A.ng, r.log10g, tg_rule(A.emission),
                     r.bg, r.wg);
-        r.n_active = 0; r.visible = 0;
+        r.n_active = 0; r.visible = 0; r.tmask = 0ull;
         row = r;
         base_s = 0;
+        tmask_s = 0ull;
     }
     __syncthreads();
     int* cl = A.cells + (size_t)rid * A.n_phi;
@@ -279,6 +282,14 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
                                             __dmul_rn(__dmul_rn(sth, sp.sin_tm), cos(__dadd_rn(phi_m, -sp.phi_m))));
                 if (cm >= sp.cos_zm) act = false;
             }
+            if (act && A.tmap) {                                  // temperature map: NaN cells do not emit (reading R24)
+                const double lT = A.tmap[(size_t)rid * A.n_phi + m];
+                act = isfinite(lT);
+                if (act) {
+                    double t;
+                    atomicOr(&tmask_s, 1ull << axis_linear(A.axT, A.nT, lT, t));
+                }
+            }
         }
         const unsigned bal = __ballot_sync(0xffffffffu, act);
         if (lane == 0) warp_cnt[w] = __popc(bal);
@@ -292,6 +303,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     }
     if (threadIdx.x == 0) {
         row.n_active = base_s;
+        row.tmask = tmask_s;
         A.rows[rid] = row;
     }
 }

@@ -1,0 +1,92 @@
+"""-m gpu: per-cell temperature maps (ppm_evaluate_map, reading R24) against the oracle."""
+import numpy as np
+import pytest
+
+import gen
+import oracle as o
+from gpu_common import make_ctx, max_rel_err, oracle_atm
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-9
+
+
+def _gpu_map(conf, tmap, ctx=None):
+    import torch
+    ctx = ctx or make_ctx(conf)
+    p = torch.as_tensor(conf["params"], dtype=torch.float64, device="cuda").contiguous()
+    tm = torch.as_tensor(np.ascontiguousarray(tmap), dtype=torch.float64, device="cuda")
+    flux, status = ctx.evaluate_map(p, tm)
+    torch.cuda.synchronize()
+    return flux.cpu().numpy(), status.cpu().numpy(), ctx
+
+
+def _smooth_map(cfg, rng, lo=5.7, hi=6.5, holes=0.1):
+    """Seeded smooth map over each spot's mesh spanning many log T intervals (node spacing 0.05), with NaN holes."""
+    ns, nt, nphi = cfg["n_spots"], cfg["n_theta"], cfg["n_phi"]
+    j = np.arange(nt)[:, None] / nt
+    m = np.arange(nphi)[None, :] / nphi
+    out = np.empty((ns, nt, nphi))
+    for s in range(ns):
+        a, b, c = rng.uniform(0, 2 * np.pi, 3)
+        f = 0.5 + 0.25 * np.sin(2 * np.pi * j + a) * np.cos(2 * np.pi * m + b) + 0.25 * np.sin(4 * np.pi * (j + m) + c)
+        out[s] = lo + (hi - lo) * f
+    out[rng.random(out.shape) < holes] = np.nan
+    return out
+
+
+@pytest.mark.parametrize("mesh", [0, 1])
+def test_smooth_map_matches_oracle(mesh):
+    conf = gen.config_c3(n_cells=36, n_phase=21, n_energy=70)
+    if mesh:
+        nside = 20
+        conf["cfg"] = dict(conf["cfg"], n_theta=4 * nside - 1, n_phi=4 * nside, mesh=1)
+    rng = np.random.default_rng(31 + mesh)
+    tmap = _smooth_map(conf["cfg"], rng)
+    g, st, ctx = _gpu_map(conf, tmap[None])
+    ref, so = o.evaluate(conf["cfg"], conf["energies"], conf["params"][0], oracle_atm(), tmap=tmap)
+    assert st[0] == 0 and so == 0 and ref.max() > 0
+    assert max_rel_err(g[0], ref) <= TOL
+    # the mask of emitting cells = geometric mask AND finite map entry (bit-exact index work)
+    mask = ctx.debug_mask()
+    nt = conf["cfg"]["n_theta"]
+    for s in range(2):
+        sp = o.spot(*conf["params"][0, 8 + 8 * s: 8 + 8 * s + 7])
+        geo = o.spot_mask_healpix(sp, conf["cfg"]["n_phi"] // 4) if mesh else o.spot_mask(sp, nt, conf["cfg"]["n_phi"])
+        assert np.array_equal(mask[s * nt:(s + 1) * nt].astype(bool), geo.astype(bool) & np.isfinite(tmap[s]))
+
+
+def test_constant_map_equals_uniform_evaluate_and_batch_of_maps():
+    import torch
+    conf = gen.config_c5(n_vec=3, n_cells=20, n_phase=12, n_energy=40)
+    ctx = make_ctx(conf)
+    p = torch.as_tensor(conf["params"], device="cuda")
+    f_uni, _ = ctx.evaluate(p)
+    cfg = conf["cfg"]
+    tmap = np.empty((3, 2, cfg["n_theta"], cfg["n_phi"]))
+    for b in range(3):
+        tmap[b, 0], tmap[b, 1] = conf["params"][b, 8 + 3], conf["params"][b, 16 + 3]
+    g, st, _ = _gpu_map(conf, tmap, ctx)
+    assert np.all(st == 0)
+    fu = f_uni.cpu().numpy()
+    for b in range(3):
+        assert max_rel_err(g[b], fu[b]) <= 1e-12
+    # temperatures below / above the table's log T axis clamp on the axis but keep their own kT and T^3 (reading R13b)
+    tmap2 = tmap.copy()
+    tmap2[:, 0] = 5.02
+    tmap2[:, 1] = 6.87
+    g2, st2, _ = _gpu_map(conf, tmap2, ctx)
+    ref, _ = o.evaluate(cfg, conf["energies"], conf["params"][1], oracle_atm(), tmap=tmap2[1])
+    assert max_rel_err(g2[1], ref) <= TOL
+    # all-NaN map: nothing emits
+    g3, st3, _ = _gpu_map(conf, np.full_like(tmap, np.nan), ctx)
+    assert np.all(st3 == 0) and np.all(g3 == 0.0)
+
+
+def test_map_mode_needs_strategy_d():
+    import paper_2510_07764_b200 as ppm
+    import torch
+    conf = gen.config_c2(n_cells=8, n_phase=8, n_energy=8)                       # emission = 1
+    ctx = make_ctx(conf)
+    tm = torch.zeros((1, 1, 8, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(ppm.PPMError):
+        ctx.evaluate_map(torch.as_tensor(conf["params"], device="cuda"), tm)
