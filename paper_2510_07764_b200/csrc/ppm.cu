@@ -208,6 +208,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->n_spots >= 1 && cfg->n_spots <= PPM_MAX_SPOTS, "n_spots must be 1..4");
     ARG(cfg->n_theta >= 1 && cfg->n_phi >= 1 && cfg->n_phase >= 1 && cfg->n_energy >= 1, "grid sizes must be >= 1");
     ARG(cfg->n_fp >= 0, "n_fp must be >= 0");
+    ARG(cfg->n_phi <= 12000, "n_phi must be <= 12000");
     ARG(cfg->emission >= 0 && cfg->emission <= 3, "emission must be 0, 1, 2 or 3");
     ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
     ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
@@ -473,7 +474,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     k_star<<<(nb + 63) / 64, 64, 0, c->stream>>>(G);
     prof_end(c);
     prof_begin(c, KID_ROWS);
-    k_rows<<<rows, 128, 0, c->stream>>>(G);
+    k_rows<<<rows, 128, tmap_dev ? sizeof(int) * (size_t)g.n_phi : 0, c->stream>>>(G);
     prof_end(c);
     prof_begin(c, KID_LOOKUP);
     k_lookup<<<rows, kNCheb * kNGL, 0, c->stream>>>(G);
@@ -776,7 +777,7 @@ extern "C" int ppm_debug_mask(ppm_ctx* c, int b, uint8_t* out)
     CK(cudaMemcpy(cl.data(), c->d_cells + (size_t)b * c->RT * nphi, sizeof(int) * cl.size(), cudaMemcpyDeviceToHost));
     std::memset(out, 0, (size_t)c->RT * nphi);
     for (int r = 0; r < c->RT; ++r)
-        for (int i = 0; i < h[r].n_active; ++i) out[(size_t)r * nphi + cl[(size_t)r * nphi + i]] = 1;
+        for (int i = 0; i < h[r].n_active; ++i) out[(size_t)r * nphi + (cl[(size_t)r * nphi + i] & 0xFFFF)] = 1;
     return PPM_OK;
 }
 

@@ -91,6 +91,7 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
         const double* MU = T + 3 * n1;
         const int* cl = A.cells + (size_t)rid * A.n_phi;
         const double* tcell = A.tmap + (size_t)rid * A.n_phi;
+        int pos = 0;                                                             // next unprocessed entry of the sorted cell list
         int node0 = -1, node1 = -1;                                              // log T node held by slice buffer 0 / 1
         for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
             const int it = __ffsll((long long)tm) - 1;                           // log T interval [it, it+1]
@@ -116,18 +117,25 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
             const double* Slo = pl ? Sb1 : Sb0;
             const double* Shi = pl ? Sb0 : Sb1;
             const double po0 = PO[0];
-            for (int base = 0; base < nact; base += 32) {
-                // ---- step A: lane <-> cell; cells of other log T intervals are skipped in this pass over the row ----
-                const int idx = base + lane;
+            // the row's list is sorted by log T interval (k_rows): the cells of interval `it` start at `pos`
+            for (bool more = true; more;) {
+                // ---- step A: lane <-> cell of this interval ----
+                const int idx = pos + lane;
                 double Fp = 0.0, pb = 0.0, tw = 0.0;
                 long long pq = 0;
                 double ww[4] = {0.0, 0.0, 0.0, 0.0};
                 int info = 0;
-                if (idx < nact) {
-                    const int m = cl[idx];
+                const int entry = (idx < nact) ? cl[idx] : -1;
+                const bool mine = (entry >= 0) && ((entry >> 16) == it);
+                const int n_mine = __popc(__ballot_sync(0xffffffffu, mine));     // a prefix of the batch (sorted list)
+                pos += n_mine;
+                more = (n_mine == 32);
+                if (mine) {
+                    const int m = entry & 0xFFFF;
                     const double lT = tcell[m];
                     double tt;
-                    if (axis_linear(TAX, A.nT, lT, tt) == it) {
+                    axis_linear(TAX, A.nT, lT, tt);
+                    {
                         const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi
                                                     : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
                         const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;

@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     for (int m0 = 0; m0 < A.n_phi; m0 += blockDim.x) {
         const int m = m0 + threadIdx.x;
         bool act = false;
+        int entry = m;                                            // temperature-map mode: m | (log T interval << 16)
         if (m < row.npix && !st.status) {
             const double dphi_m = (A.mesh == 1) ? __dadd_rn(__dadd_rn(row.phi0, __dmul_rn((double)m, row.dphi)), -sp.phi_c)
                                                 : __dadd_rn(-sp.W, __dmul_rn((double)m + 0.5, sp.dphi));
@@ -287,7 +288,9 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
                 act = isfinite(lT);
                 if (act) {
                     double t;
-                    atomicOr(&tmask_s, 1ull << axis_linear(A.axT, A.nT, lT, t));
+                    const int iT = axis_linear(A.axT, A.nT, lT, t);
+                    atomicOr(&tmask_s, 1ull << iT);
+                    entry = m | (iT << 16);
                 }
             }
         }
@@ -296,10 +299,35 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         __syncthreads();
         int off = base_s;
         for (int ww = 0; ww < w; ++ww) off += warp_cnt[ww];
-        if (act) cl[off + __popc(bal & ((1u << lane) - 1u))] = m;
+        if (act) cl[off + __popc(bal & ((1u << lane) - 1u))] = entry;
         __syncthreads();
         if (threadIdx.x == 0) base_s += warp_cnt[0] + warp_cnt[1] + warp_cnt[2] + warp_cnt[3];
         __syncthreads();
+    }
+    if (A.tmap && tmask_s) {
+        // temperature-map mode: stable sort of the row's list by log T interval (ordered compaction per interval through
+        // a shared-memory copy), so that k_cells_map finds the cells of each interval in one contiguous, ordered range
+        extern __shared__ int tmp_cells[];
+        const int n = base_s;
+        for (int i = threadIdx.x; i < n; i += blockDim.x) tmp_cells[i] = cl[i];
+        if (threadIdx.x == 0) base_s = 0;
+        __syncthreads();
+        for (unsigned long long tm = tmask_s; tm; tm &= tm - 1) {
+            const int it = __ffsll((long long)tm) - 1;
+            for (int i0 = 0; i0 < n; i0 += blockDim.x) {
+                const int i = i0 + threadIdx.x;
+                const bool take = (i < n) && ((tmp_cells[i] >> 16) == it);
+                const unsigned bal = __ballot_sync(0xffffffffu, take);
+                if (lane == 0) warp_cnt[w] = __popc(bal);
+                __syncthreads();
+                int off = base_s;
+                for (int ww = 0; ww < w; ++ww) off += warp_cnt[ww];
+                if (take) cl[off + __popc(bal & ((1u << lane) - 1u))] = tmp_cells[i];
+                __syncthreads();
+                if (threadIdx.x == 0) base_s += warp_cnt[0] + warp_cnt[1] + warp_cnt[2] + warp_cnt[3];
+                __syncthreads();
+            }
+        }
     }
     if (threadIdx.x == 0) {
         row.n_active = base_s;
