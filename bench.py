@@ -188,6 +188,8 @@ def main():
     ap.add_argument("--workload", default="C5", choices=["C5", "T", "C2", "C3", "C4"])
     ap.add_argument("--batch", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tmap", type=float, default=None, metavar="DEX",
+                    help="per-cell temperature maps (ppm_evaluate_map): each spot's log T modulated by +-DEX over its mesh")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1],
                     help="0: fp64 everywhere (default, the judged path); 1: fp32 interpolation + exponential")
     args = ap.parse_args()
@@ -234,13 +236,26 @@ def main():
     st_host = np.empty((B,), dtype=np.int32)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
+    tmap = None
+    if args.tmap is not None:
+        tmap = torch.as_tensor(gen.smooth_temperature_map(cfg, conf["params"], args.tmap), device=dev).contiguous()
+
     def step():
-        ctx.evaluate(params, flux, status)
+        if tmap is not None:
+            ctx.evaluate_map(params, tmap, flux, status)
+        else:
+            ctx.evaluate(params, flux, status)
         ctx.fold_response(flux, params, counts)
         ctx.loglike(counts, data, bkg, exposure, ll)
 
     def step_e2e():
-        ctx.loglike_host(params_pinned.numpy(), data, bkg, exposure, ll_host, st_host)
+        if tmap is not None:               # no host-buffer entry for maps: device-pointer calls + explicit copies
+            params.copy_(params_pinned, non_blocking=True)
+            step()
+            ll_host[:] = ll.cpu().numpy()
+            st_host[:] = status.cpu().numpy()
+        else:
+            ctx.loglike_host(params_pinned.numpy(), data, bkg, exposure, ll_host, st_host)
 
     def sync():
         torch.cuda.synchronize()
@@ -299,10 +314,12 @@ def main():
             peak_dfma = None
         kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
         table = bool(cfg["emission"])
-        roofline = {"bound": "alu", "kernel": "k_cells_tab" if table else "k_cells_bb", "achieved": achieved,
+        default_kernel = table and args.tmap is None and args.precision == 0
+        roofline = {"bound": "alu", "kernel": ("k_cells_map" if args.tmap is not None else "k_cells_tab32" if args.precision else "k_cells_tab")
+                    if table else "k_cells_bb", "achieved": achieved,
                     "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
-                    "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                    "executed_flop_per_unit": EXECUTED_FLOP_PER_TRIPLE if table else None,
+                    "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if default_kernel else None,
+                    "executed_flop_per_unit": EXECUTED_FLOP_PER_TRIPLE if default_kernel else None,
                     "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
                                    "Roofline); MEASURED_PEAKS.json has no FP64 entry",
                     "peak_measured_dfma_chain": peak_dfma,
@@ -313,7 +330,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_eval": ms_per_step / B,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 0 else "f32 interpolation / f64 geometry+sums", "data": "synthetic",
-                "config": {"workload": desc, "name": args.workload, "precision": args.precision, "batch_per_gpu": B, "n_fp": ctx.n_fp,
+                "config": {"workload": desc, "name": args.workload, "precision": args.precision, "tmap_dex": args.tmap, "batch_per_gpu": B, "n_fp": ctx.n_fp,
                            "l2": "flushed before every step (256 MiB write between the steps' CUDA-event brackets)",
                            "step": "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params_pinned.numel() * 8),

@@ -251,3 +251,21 @@ def synthetic_counts(n_phase, n_channel, total=1.0e6, bkg_frac=0.05, seed=SEED0 
     bkg = np.full(n_channel, bkg_frac * total / (n_phase * n_channel))
     data = rng.poisson(m + bkg[None, :]).astype(np.float64)
     return data, bkg
+
+
+def smooth_temperature_map(cfg, params, amplitude=0.05, seed=SEED0 + 9):
+    """Seeded smooth per-cell temperature maps log10 T[B][n_spots][n_theta][n_phi] for ppm_evaluate_map: each spot's own
+    log10 T (params) modulated over its mesh by +- `amplitude` dex of low-order structure (the paper's maps come from a
+    physical surface-heating model, which is not available; the table's log T node spacing is 0.05 dex,
+    so amplitude 0.05 spans 2-3 intervals per row and 0.3 about a dozen).  No NaN holes."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    B = params.shape[0]
+    ns, nt, nphi = cfg["n_spots"], cfg["n_theta"], cfg["n_phi"]
+    j = np.arange(nt, dtype=np.float64)[:, None] / nt
+    m = np.arange(nphi, dtype=np.float64)[None, :] / nphi
+    out = np.empty((B, ns, nt, nphi))
+    for b in range(B):
+        for s in range(ns):
+            a, c = rng.uniform(0.0, 2.0 * np.pi, size=2)
+            out[b, s] = params[b, 8 + 8 * s + 3] + amplitude * np.sin(2.0 * np.pi * j + a) * np.cos(2.0 * np.pi * m + c)
+    return out

@@ -222,20 +222,35 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
                     }
                     __syncwarp();
                     const double2* KAq = KA + (1 - jlo);
-                    const bool clampc = inf & 0x8000;
+                    if (!(inf & 0x8000)) {
 #pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        long long s = q + uef[i];
-                        if (clampc) s = s < 0 ? 0 : (s > s_top ? s_top : s);     // reading R13b
-                        const int shi = (int)(s >> 32);
-                        const double2* kp = KAq + (shi >> 20);
-                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
-                        const double2 c01 = kp[0], c23 = kp[KW];
-                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
-                        const double r = y + kMagic;
-                        const int n = __double2loint(r);
-                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        if (n >= -1000) acc[i] += val;
+                        for (int i = 0; i < EPL; ++i) {
+                            const long long s = q + uef[i];
+                            const int shi = (int)(s >> 32);
+                            const double2* kp = KAq + (shi >> 20);
+                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                            const double2 c01 = kp[0], c23 = kp[KW];
+                            const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+                            const double r = y + kMagic;
+                            const int n = __double2loint(r);
+                            const double val = exp2_frac_scaled(y - (r - kMagic), n);
+                            if (n >= -1000) acc[i] += val;
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < EPL; ++i) {
+                            long long s = q + uef[i];
+                            s = s < 0 ? 0 : (s > s_top ? s_top : s);             // clamp to the table (reading R13b)
+                            const int shi = (int)(s >> 32);
+                            const double2* kp = KAq + (shi >> 20);
+                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                            const double2 c01 = kp[0], c23 = kp[KW];
+                            const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+                            const double r = y + kMagic;
+                            const int n = __double2loint(r);
+                            const double val = exp2_frac_scaled(y - (r - kMagic), n);
+                            if (n >= -1000) acc[i] += val;
+                        }
                     }
                 }
             }
