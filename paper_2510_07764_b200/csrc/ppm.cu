@@ -439,21 +439,21 @@ static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, 
 }
 
 // shared memory of k_cells_map with `nw` warps (ppm_cells_map.cuh layout)
-static size_t cells_map_smem(const ppm_ctx* c, int nw)
+static size_t cells_map_smem(const ppm_ctx* c, int nw, int wst)
 {
-    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 16) + 2 * (size_t)c->nmu * c->nx +
+    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 16) + 2 * (size_t)c->nmu * wst +
                              4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT);
 }
 
-template <int EPL>
+template <int EPL, bool WIN>
 static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
     switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_map<EPL, 1>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_map<EPL, 3>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_map<EPL, 5>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_map<EPL, 7>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_map<EPL, 9>, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_map<EPL, 9, WIN>, a, grid, threads, smem);
     }
 }
 
@@ -510,23 +510,50 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     int rc;
     if (tmap_dev) {
-        // temperature-map mode: two FP64 node slices in shared memory -> fewer warps (output phases) per block
+        // temperature-map mode: two FP64 log T node slices in shared memory.  Full-width slices leave room for 8 warps;
+        // slices cut to the logx columns a row's interval can reach (wst columns) leave room for 16.  Both kernels are
+        // launched, each row is taken by the windowed one if all its intervals fit wst columns, else by the full-width one.
+        A.tmap = tmap_dev; A.values = c->d_values; A.axT = c->d_axT; A.nT = c->nT; A.ng = c->ng;
         int nwm = 0;
-        for (int v : {8, 6, 4, 2, 1}) if (cells_map_smem(c, v) <= 227 * 1024) { nwm = v; break; }
+        for (int v : {8, 6, 4, 2, 1}) if (cells_map_smem(c, v, c->nx) <= 227 * 1024) { nwm = v; break; }
         if (!nwm) { set_err("temperature-map mode: table and template do not fit in shared memory"); return PPM_ERR_ARG; }
         nwm = std::min(nwm, g.n_phase);
-        A.nw = nwm;
-        A.tmap = tmap_dev; A.values = c->d_values; A.axT = c->d_axT; A.nT = c->nT; A.ng = c->ng;
-        dim3 grid(c->nchunk, (g.n_phase + nwm - 1) / nwm, nb * c->n_etile);
-        const size_t smem_map = cells_map_smem(c, nwm);
+        int wst = 0;
+        if (g.n_phase >= 16) {
+            const long budget = 227 * 1024 / 8 - (long)cells_map_smem(c, 16, 0) / 8;
+            wst = (int)std::min<long>(c->nx, budget > 0 ? budget / (2 * c->nmu) : 0);
+            if (wst < c->wmax + 12 || wst >= c->nx) wst = 0;                       // too narrow to be useful / nothing to gain
+        }
+        A.wst = wst; A.map_split = wst ? 1 : 0;
         prof_begin(c, KID_CELLS);
-        switch (c->epl) {
-        case 1:  rc = dispatch_cells_map<1>(c, A, grid, nwm * 32, smem_map); break;
-        case 2:  rc = dispatch_cells_map<2>(c, A, grid, nwm * 32, smem_map); break;
-        case 4:  rc = dispatch_cells_map<4>(c, A, grid, nwm * 32, smem_map); break;
-        case 5:  rc = dispatch_cells_map<5>(c, A, grid, nwm * 32, smem_map); break;
-        case 8:  rc = dispatch_cells_map<8>(c, A, grid, nwm * 32, smem_map); break;
-        default: rc = dispatch_cells_map<10>(c, A, grid, nwm * 32, smem_map); break;
+        rc = PPM_OK;
+        if (wst) {
+            CellArgs W = A;
+            W.nw = 16;
+            dim3 gridw(c->nchunk, (g.n_phase + 15) / 16, nb * c->n_etile);
+            const size_t smw = cells_map_smem(c, 16, wst);
+            switch (c->epl) {
+            case 1:  rc = dispatch_cells_map<1, true>(c, W, gridw, 512, smw); break;
+            case 2:  rc = dispatch_cells_map<2, true>(c, W, gridw, 512, smw); break;
+            case 4:  rc = dispatch_cells_map<4, true>(c, W, gridw, 512, smw); break;
+            case 5:  rc = dispatch_cells_map<5, true>(c, W, gridw, 512, smw); break;
+            case 8:  rc = dispatch_cells_map<8, true>(c, W, gridw, 512, smw); break;
+            default: rc = dispatch_cells_map<10, true>(c, W, gridw, 512, smw); break;
+            }
+            c->launches += 1;
+        }
+        if (!rc) {
+            A.nw = nwm;
+            dim3 grid(c->nchunk, (g.n_phase + nwm - 1) / nwm, nb * c->n_etile);
+            const size_t smem_map = cells_map_smem(c, nwm, c->nx);
+            switch (c->epl) {
+            case 1:  rc = dispatch_cells_map<1, false>(c, A, grid, nwm * 32, smem_map); break;
+            case 2:  rc = dispatch_cells_map<2, false>(c, A, grid, nwm * 32, smem_map); break;
+            case 4:  rc = dispatch_cells_map<4, false>(c, A, grid, nwm * 32, smem_map); break;
+            case 5:  rc = dispatch_cells_map<5, false>(c, A, grid, nwm * 32, smem_map); break;
+            case 8:  rc = dispatch_cells_map<8, false>(c, A, grid, nwm * 32, smem_map); break;
+            default: rc = dispatch_cells_map<10, false>(c, A, grid, nwm * 32, smem_map); break;
+            }
         }
     } else {
         dim3 grid(c->nchunk, c->npg, nb * c->n_etile);

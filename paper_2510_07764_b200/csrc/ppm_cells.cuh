@@ -21,6 +21,8 @@ struct CellArgs {
     const double* values;    // temperature-map mode: the 4-D table [nT][ng][nmu][nx]
     const double* axT;       // temperature-map mode: log T axis [nT]
     int nT, ng;
+    int wst, map_split;      // temperature-map mode: column capacity of the windowed slice buffers; 1 = rows are split
+                             // between the windowed (16-warp) and the full-width (8-warp) launch
     unsigned long long* pairs;   // counter: (cell, phase) pairs with F_p != 0 (energy tile 0 only)
     double x0_over_h, inv_h;
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;

@@ -9,7 +9,8 @@
 // intervals in ascending order; for interval iT it stages the node slices iT and iT+1 -- blended over the row's two
 // log g nodes on the fly from the L2-resident 4-D table -- into two shared-memory buffers (the upper node of one
 // interval is the lower node of the next: ping-pong, one new slice per step), and processes the row's cells of that
-// interval.  Two FP64 slices take 178 KB, so a block has 8 warps (8 output phases) instead of 16.
+// interval.  Two full-width FP64 slices take 178 KB (room for 8 warps only); the WIN variant cuts the slices to the
+// logx columns the interval's pairs can reach (map_window) and keeps 16 warps.
 // Everything per pair and per triple is k_cells_tab's scheme (fixed-point logx coordinate, fused shuffle pass to
 // per-interval monomial coefficients, Horner + degree-8 exp2), with T, kT and T^3 taken per cell.
 #pragma once
@@ -22,8 +23,39 @@ __device__ __forceinline__ double contract4(const double* __restrict__ sp0, int 
     return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
 }
 
-template <int EPL, int NPL>
-__global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
+// logx node window [c_lo, c_hi] that bounds every pair of log T interval `it` of a row: u = (log10(z E / kT) - x0) / h
+// over z in [zlo, zhi] (template), E in [E_first, E_last] (energy tile, as fixed-point uef) and log T in the part of the
+// row's range [tmin, tmax] that lies in the interval (temperatures outside the axis fall in the first / last interval).
+// One node of slack on each side beyond the stencil's reach (c - 1 .. c + 2).
+__device__ inline void map_window(const RowD& row, const double* __restrict__ axT, int nT, int it, double inv_h,
+                                  double x0_over_h, double ue_first, double ue_last, int nx, int& c_lo, int& c_hi)
+{
+    const int first = __ffsll((long long)row.tmask) - 1, last = 63 - __clzll((long long)row.tmask);
+    const double t_lo = (it == first) ? fmin(row.tmin, axT[it]) : axT[it];
+    const double t_hi = (it == last) ? fmax(row.tmax, axT[imin_(it + 1, nT - 1)]) : axT[it + 1];
+    const double log10kB = log10(kKB_keV_K);
+    const double u_lo = (log10(row.zlo) - (log10kB + t_hi)) * inv_h - x0_over_h + ue_first;
+    const double u_hi = (log10(row.zhi) - (log10kB + t_lo)) * inv_h - x0_over_h + ue_last;
+    c_lo = imin_(imax_((int)floor(fmax(u_lo, -4.0)) - 2, 0), nx - 1);
+    c_hi = imin_(imax_((int)floor(fmin(u_hi, (double)nx + 4.0)) + 3, 0), nx - 1);
+}
+
+// does every interval of the row fit a window of `wst` columns?  (rows that do not are left to the full-width kernel)
+__device__ inline bool map_row_fits(const RowD& row, const double* __restrict__ axT, int nT, double inv_h, double x0_over_h,
+                                    double ue_first, double ue_last, int nx, int wst)
+{
+    for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
+        int c_lo, c_hi;
+        map_window(row, axT, nT, __ffsll((long long)tm) - 1, inv_h, x0_over_h, ue_first, ue_last, nx, c_lo, c_hi);
+        if (c_hi - c_lo + 1 > wst) return false;
+    }
+    return true;
+}
+
+// WIN = true: 16 warps, the two node slices hold only the window's columns (row stride A.wst); rows whose windows do not
+// fit are skipped (the WIN = false launch takes them).  WIN = false: 8 warps, full-width slices (row stride nx).
+template <int EPL, int NPL, bool WIN>
+__global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -34,7 +66,8 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
     const int e0 = et * 32 * EPL;
     const int n1 = A.n_fp + 1;
     const int nx = A.nx;
-    const int plane = A.nmu * nx;
+    const int wst = WIN ? A.wst : nx;                                           // row stride of the slice buffers
+    const int plane = A.nmu * wst;
     // shared layout (doubles): per warp { KA [KW], KB [KW], R0 (q, qb), R1 (v0, v1), R2 (v2, v3), R3 (1-t, t) [32] as
     // double2, RI [32] int } | S0 [nmu][nx] | S1 [nmu][nx] | T [4][n1] | MUAX [nmu] | TAX [nT]
     constexpr int KW = 32 * NPL;
@@ -63,6 +96,7 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
     const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
     const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
     const long long s_top = ((long long)(nx - 1) << 52) - 1;
+    const double ue_first = (double)uef_first / kTwo52, ue_last = (double)uef_last / kTwo52;
     for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
     for (int i = threadIdx.x; i < A.nT; i += blockDim.x) TAX[i] = A.axT[i];
 
@@ -79,6 +113,10 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
         const RowD& row = A.rows[rid];
         const int nact = row.n_active;
         if (nact == 0 || !row.visible) continue;
+        if (A.map_split) {                                                       // each row belongs to exactly one launch
+            const bool fits = map_row_fits(row, A.axT, A.nT, A.inv_h, A.x0_over_h, ue_first, ue_last, nx, A.wst);
+            if (fits != WIN) continue;
+        }
         const SpotD& sp = A.spots[rid / A.n_theta];
         __syncthreads();
         {
@@ -95,21 +133,26 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
         int node0 = -1, node1 = -1;                                              // log T node held by slice buffer 0 / 1
         for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
             const int it = __ffsll((long long)tm) - 1;                           // log T interval [it, it+1]
-            const int pl = (node1 == it) ? 1 : 0;
+            int c_lo = 0, c_hi = nx - 1;
+            if (WIN) map_window(row, A.axT, A.nT, it, A.inv_h, A.x0_over_h, ue_first, ue_last, nx, c_lo, c_hi);
+            const int pl = (!WIN && node1 == it) ? 1 : 0;                        // windowed buffers are interval-specific: no reuse
             __syncthreads();                                                     // readers of the previous interval are done
 #pragma unroll
             for (int h = 0; h < 2; ++h) {                                        // h = 0: lower node -> buffer pl; 1: upper -> 1 - pl
                 const int buf = h ? 1 - pl : pl, node = it + h;
-                if ((buf ? node1 : node0) == node) continue;
+                if (!WIN && (buf ? node1 : node0) == node) continue;
                 if (buf) node1 = node; else node0 = node;
                 double* dst = buf ? Sb1 : Sb0;
-                const double* src = A.values + ((size_t)node * A.ng + row.bg) * plane;
-                for (int i = threadIdx.x; i < plane; i += blockDim.x) {
+                const double* src = A.values + ((size_t)node * A.ng + row.bg) * ((size_t)A.nmu * nx);
+                const int wcols = WIN ? c_hi - c_lo + 1 : nx;
+                for (int i = threadIdx.x; i < A.nmu * wcols; i += blockDim.x) {
+                    const int mu_i = i / wcols, col = i - mu_i * wcols;
+                    const size_t gi = (size_t)mu_i * nx + (WIN ? c_lo : 0) + col;
                     double v = 0.0;
 #pragma unroll
                     for (int gq = 0; gq < 4; ++gq)
-                        if (row.wg[gq] != 0.0) v = fma(row.wg[gq], __ldg(src + (size_t)gq * plane + i), v);
-                    dst[i] = v;
+                        if (row.wg[gq] != 0.0) v = fma(row.wg[gq], __ldg(src + (size_t)gq * A.nmu * nx + gi), v);
+                    dst[mu_i * wst + col] = v;
                 }
             }
             __syncthreads();
@@ -162,7 +205,7 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
                             const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
                             const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
                             const int clamped = (sa < 0) || (sb2 > s_top);
-                            info = (mb * nx) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
+                            info = mb | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
                         }
                     }
                 }
@@ -186,13 +229,13 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
                     const long long q = __double_as_longlong(r0.x);
                     const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                     const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
-                    const int soff = (inf & 0x7FFF) + jlo - 1 + NPL * lane;
+                    const int soff = (inf & 0x7FFF) * wst - c_lo + jlo - 1 + NPL * lane;
                     const int n0 = jlo - 1 + NPL * lane;
                     double f[NPL + 3];
 #pragma unroll
                     for (int jn = 0; jn < NPL; ++jn)
-                        f[1 + jn] = fma(r3.y, contract4(Shi + soff + jn, nx, v0, v1, v2, v3),
-                                        fma(r3.x, contract4(Slo + soff + jn, nx, v0, v1, v2, v3), qb));
+                        f[1 + jn] = fma(r3.y, contract4(Shi + soff + jn, wst, v0, v1, v2, v3),
+                                        fma(r3.x, contract4(Slo + soff + jn, wst, v0, v1, v2, v3), qb));
                     f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
                     if (NPL == 1) {
                         f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
@@ -262,7 +305,10 @@ __global__ void __launch_bounds__(256, 1) k_cells_map(CellArgs A)
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
             const int e = e0 + lane + 32 * i;
-            if (e < A.nE) out[e] = acc[i] / A.en[e];                            // the 1/E_e of Eq 47
+            if (e < A.nE) {                                                      // the 1/E_e of Eq 47
+                const double v = acc[i] / A.en[e];
+                out[e] = (!WIN && A.map_split) ? out[e] + v : v;                   // the full-width launch runs second and adds
+            }
         }
     }
 }

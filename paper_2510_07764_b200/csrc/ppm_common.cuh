@@ -49,6 +49,8 @@ struct RowD {
     int bg, n_active, visible, npix;              // npix: azimuth cells of this row (HEALPix rings differ)
     double phi0, dphi;                            // azimuth of cell m: phi0 + m dphi (HEALPix mesh only)
     unsigned long long tmask;                     // temperature-map mode: bit i set iff an active cell lies in log T interval i
+    double tmin, tmax;                            // temperature-map mode: range of log10 T over the row's emitting cells
+    double zlo, zhi;                              // range of the template's redshift factor z over the fine phases
 };
 
 __host__ __device__ inline int imin_(int a, int b) { return a < b ? a : b; }

@@ -197,6 +197,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     __shared__ int warp_cnt[4];
     __shared__ int base_s;
     __shared__ unsigned long long tmask_s;
+    __shared__ double tlo_s[4], thi_s[4];
     const int rid = blockIdx.x;                          // (b * n_spots + s) * n_theta + j
     const int j = rid % A.n_theta, bs = rid / A.n_theta, b = bs / A.n_spots;
     const StarD st = A.stars[b];
@@ -259,7 +260,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         if (A.emission != PPM_EMISSION_BLACKBODY && !st.status)
             axis_w4(A.axg, A.ng, r.log10g, tg_rule(A.emission),
                     r.bg, r.wg);
-        r.n_active = 0; r.visible = 0; r.tmask = 0ull;
+        r.n_active = 0; r.visible = 0; r.tmask = 0ull; r.tmin = r.tmax = r.zlo = r.zhi = 0.0;
         row = r;
         base_s = 0;
         tmask_s = 0ull;
@@ -268,6 +269,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     int* cl = A.cells + (size_t)rid * A.n_phi;
     const double ct = cos(row.theta), sth = sin(row.theta);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double tlo = INFINITY, thi = -INFINITY;
     for (int m0 = 0; m0 < A.n_phi; m0 += blockDim.x) {
         const int m = m0 + threadIdx.x;
         bool act = false;
@@ -291,6 +293,7 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
                     const int iT = axis_linear(A.axT, A.nT, lT, t);
                     atomicOr(&tmask_s, 1ull << iT);
                     entry = m | (iT << 16);
+                    tlo = fmin(tlo, lT); thi = fmax(thi, lT);
                 }
             }
         }
@@ -304,6 +307,13 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
         if (threadIdx.x == 0) base_s += warp_cnt[0] + warp_cnt[1] + warp_cnt[2] + warp_cnt[3];
         __syncthreads();
     }
+#pragma unroll
+    for (int q = 16; q > 0; q >>= 1) {
+        tlo = fmin(tlo, __shfl_xor_sync(0xffffffffu, tlo, q));
+        thi = fmax(thi, __shfl_xor_sync(0xffffffffu, thi, q));
+    }
+    if (lane == 0) { tlo_s[w] = tlo; thi_s[w] = thi; }
+    __syncthreads();
     if (A.tmap && tmask_s) {
         // temperature-map mode: stable sort of the row's list by log T interval (ordered compaction per interval through
         // a shared-memory copy), so that k_cells_map finds the cells of each interval in one contiguous, ordered range
@@ -332,6 +342,8 @@ __global__ void __launch_bounds__(128) k_rows(GeoArgs A)
     if (threadIdx.x == 0) {
         row.n_active = base_s;
         row.tmask = tmask_s;
+        row.tmin = fmin(fmin(tlo_s[0], tlo_s[1]), fmin(tlo_s[2], tlo_s[3]));
+        row.tmax = fmax(fmax(thi_s[0], thi_s[1]), fmax(thi_s[2], thi_s[3]));
         A.rows[rid] = row;
     }
 }
@@ -485,7 +497,23 @@ __global__ void __launch_bounds__(128) k_template(GeoArgs A)
     __syncthreads();
     double* out = A.tmpl + (size_t)rid * 4 * n1;
     for (int i = threadIdx.x; i < 4 * n1; i += blockDim.x) out[i] = F[i];
-    if (threadIdx.x == 0) A.rows[rid].visible = visible_ring;
+    // range of z over the fine phases (after the fill): bounds every z_p of Eq 46; used to size logx windows
+    __shared__ double zlo_s[4], zhi_s[4];
+    double zlo = INFINITY, zhi = -INFINITY;
+    if (visible_ring)
+        for (int i = threadIdx.x; i < n1; i += blockDim.x) { zlo = fmin(zlo, Z[i]); zhi = fmax(zhi, Z[i]); }
+#pragma unroll
+    for (int q = 16; q > 0; q >>= 1) {
+        zlo = fmin(zlo, __shfl_xor_sync(0xffffffffu, zlo, q));
+        zhi = fmax(zhi, __shfl_xor_sync(0xffffffffu, zhi, q));
+    }
+    if ((threadIdx.x & 31) == 0) { zlo_s[threadIdx.x >> 5] = zlo; zhi_s[threadIdx.x >> 5] = zhi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        A.rows[rid].visible = visible_ring;
+        A.rows[rid].zlo = fmin(fmin(zlo_s[0], zlo_s[1]), fmin(zlo_s[2], zlo_s[3]));
+        A.rows[rid].zhi = fmax(fmax(zhi_s[0], zhi_s[1]), fmax(zhi_s[2], zhi_s[3]));
+    }
 }
 
 }  // namespace ppm

@@ -90,3 +90,18 @@ def test_map_mode_needs_strategy_d():
     tm = torch.zeros((1, 1, 8, 8), dtype=torch.float64, device="cuda")
     with pytest.raises(ppm.PPMError):
         ctx.evaluate_map(torch.as_tensor(conf["params"], device="cuda"), tm)
+
+
+def test_rows_split_between_the_windowed_and_the_full_width_launch():
+    """Temperatures far outside the table's log T axis keep their own kT (reading R13b), which moves the row's logx
+    window by tens of columns: such rows do not fit the windowed slice buffers and go to the full-width launch, the
+    others to the windowed one; the two launches add into the same tiles."""
+    conf = gen.config_c3(n_cells=30, n_phase=32, n_energy=64)
+    cfg = conf["cfg"]
+    rng = np.random.default_rng(77)
+    tmap = _smooth_map(cfg, rng, lo=5.9, hi=6.3, holes=0.05)
+    tmap[0, 4:9, ::3] = 4.2                       # 0.9 dex below the axis: window wider than the buffers
+    tmap[1, 20:24, 1::2] = 7.6                    # 0.8 dex above
+    g, st, _ = _gpu_map(conf, tmap[None])
+    ref, so = o.evaluate(cfg, conf["energies"], conf["params"][0], oracle_atm(), tmap=tmap)
+    assert st[0] == 0 and so == 0 and max_rel_err(g[0], ref) <= TOL
