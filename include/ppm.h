@@ -18,6 +18,8 @@
  *     torch.cuda.current_stream().cuda_stream, or NULL for the default stream).  Calls that
  *     take only device pointers are asynchronous and never synchronise; ppm_create,
  *     ppm_load_atmosphere, ppm_set_response, ppm_*_host and ppm_debug_* synchronise the stream.
+ *     After one warm-up call (lazy scratch allocation) the device-pointer calls allocate nothing, so a whole step
+ *     (ppm_evaluate + ppm_fold_response + ppm_loglike) can be captured into a CUDA graph on that stream and replayed.
  *   - One context per stream; a context is not thread-safe.
  *   - Return value: 0 on success, a negative PPM_ERR_* otherwise; ppm_last_error() gives text.
  *   - Per-vector physics failures do not fail the call: status[b] carries the bits below,

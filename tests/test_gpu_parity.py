@@ -347,3 +347,38 @@ def test_random_prior_vectors_sweep():
         for b, (ref, so) in enumerate(refs):
             assert st[b] == so == 0
             assert max_rel_err(g[b], ref) <= tol, (precision, b)
+
+
+def test_step_is_capturable_in_a_cuda_graph():
+    """The device-pointer calls neither synchronise nor allocate after their first use: evaluate + fold + ln L can be
+    captured into a CUDA graph on the context's stream and replayed, bit-identical to the eager run."""
+    import torch
+    conf = gen.config_c5(n_vec=2, n_cells=24, n_phase=16, n_energy=300)
+    rsp = gen.synthetic_response(conf["energies"])
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = make_ctx(conf)
+        ctx.set_response(rsp["n_channel"], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"])
+        p = torch.as_tensor(conf["params"], device="cuda")
+        d_h, b_h = gen.synthetic_counts(16, rsp["n_channel"])
+        data, bkg = torch.as_tensor(d_h, device="cuda"), torch.as_tensor(b_h, device="cuda")
+        flux = torch.empty((2, 16, 300), dtype=torch.float64, device="cuda")
+        st = torch.empty((2,), dtype=torch.int32, device="cuda")
+        counts = torch.empty((2, 16, rsp["n_channel"]), dtype=torch.float64, device="cuda")
+        ll = torch.empty((2,), dtype=torch.float64, device="cuda")
+
+        def step():
+            ctx.evaluate(p, flux, st)
+            ctx.fold_response(flux, p, counts)
+            ctx.loglike(counts, data, bkg, 1.0e6, ll)
+        step()
+        torch.cuda.synchronize()
+        ref = ll.clone()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            step()
+        ll.zero_()
+        flux.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(ll, ref) and bool(torch.isfinite(ll).all()) and float(flux.max()) > 0
