@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ppm|reference]
                     [--workload C5|T|C2|C3|C4] [--batch B] [--no-cpu-baseline]
+                    [--precision 0|1] [--tmap DEX]
 
 A *step* is one pass of the whole hot path S0..S7 over one batch of B seeded
 parameter vectors: ppm_evaluate -> ppm_fold_response -> ppm_loglike, everything through the C ABI of
@@ -18,6 +19,9 @@ ppm_loglike_host (host parameter buffer in, host ln L out, copies inside the tim
 accumulated (cell, phase, energy) triple / the kernel's own
 CUDA-event time measured inside the library on its launch stream.  `cpu_baseline` times the CPU
 oracle as it stands on a bounded sample of the same workload (rank 0, N = 1 only).
+
+--precision 1 times the FP32-interpolation variant (tolerance 1e-4 instead of 1e-9; not the judged path), --tmap DEX the
+per-cell temperature-map entry ppm_evaluate_map with a seeded smooth map of +-DEX around each spot's log T.
 
 --impl reference: there is no reference implementation (the paper's code is not available); per
 the task contract the reference arm is the CPU oracle, timed on the host cores on a bounded sample.
