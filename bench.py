@@ -319,13 +319,16 @@ def main():
         kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
         table = bool(cfg["emission"])
         default_kernel = table and args.tmap is None and args.precision == 0
+        # precision = 1 runs the per-triple work on the FP32 pipe: 128 FFMA lanes per SM, twice the FP64 figure
+        peak_nominal = FP64_NOMINAL_TFLOPS * (2.0 if args.precision == 1 else 1.0)
         roofline = {"bound": "alu", "kernel": ("k_cells_map" if args.tmap is not None else "k_cells_tab32" if args.precision else "k_cells_tab")
                     if table else "k_cells_bb", "achieved": achieved,
-                    "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+                    "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
                     "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if default_kernel else None,
                     "executed_flop_per_unit": EXECUTED_FLOP_PER_TRIPLE if default_kernel else None,
-                    "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
-                                   "Roofline); MEASURED_PEAKS.json has no FP64 entry",
+                    "peak_source": ("nominal FP32 FMA pipe: 148 SM x 128 FFMA/clk x 2 flop x 1.965 GHz" if args.precision == 1 else
+                                    "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
+                                    "Roofline); MEASURED_PEAKS.json has no FP64 entry"),
                     "peak_measured_dfma_chain": peak_dfma,
                     "frac_of_measured_dfma_chain": (achieved / peak_dfma) if peak_dfma else None,
                     "flop_per_unit": FLOP_PER_TRIPLE, "units_per_launch": tri_per_launch,
