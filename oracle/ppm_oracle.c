@@ -17,7 +17,9 @@
  *
  * Arithmetic: IEEE double everywhere, long double inside the quadrature / root solve.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P16 of DESIGN.md.  Parts that have
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P20 of DESIGN.md (P17-P20, tests/test_oracle_rotation.py: the
+ * rotation / aberration terms of the template against a moving blackbody in flat space and against unit vectors,
+ * the Eq 41-44 fill, Eq 10's Obar^6 terms).  Parts that have
  * no pin other than internal consistency are listed under "parity unpinned" there:
  *   - absolute agreement with the external NICER-grade benchmarks (OS1a-l, Ring/Crescent)
  *     -- PARITY UNPINNED (reference data not available).
