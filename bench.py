@@ -2,7 +2,7 @@
 """bench.py -- throughput of the PPM hot path (pulse-profile evaluations per second).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ppm|reference]
-                    [--workload C5|T|C2|C3|C4] [--batch B] [--no-cpu-baseline]
+                    [--workload C5|T|C1|C2|C3|C4] [--batch B] [--no-cpu-baseline | --cpu-baseline sample|full]
                     [--precision 0|1] [--tmap DEX]
 
 A *step* is one pass of the whole hot path S0..S7 over one batch of B seeded
@@ -15,10 +15,15 @@ units, no data-path collective ("scaling": "weak"); the time is the max over ran
 
 One JSON line is printed by rank 0.  `value` has the parameter batch resident in HBM; `e2e` runs
 ppm_loglike_host (host parameter buffer in, host ln L out, copies inside the timed region).
-`roofline` is for the dominant kernel k_cells: bound "alu" (FP64 pipe), algorithmic flops = 86 per
-accumulated (cell, phase, energy) triple / the kernel's own
-CUDA-event time measured inside the library on its launch stream.  `cpu_baseline` times the CPU
-oracle as it stands on a bounded sample of the same workload (rank 0, N = 1 only).
+`roofline` is for the dominant kernel k_cells: bound "alu" (FP64 pipe).  `achieved` / `frac` count the FP64
+flop the kernel EXECUTES per launch (2 DFMA + DADD + DMUL thread instructions from the ncu capture of this very
+workload and kernel source, paper_2510_07764_b200/ncu_captured.json; null when no capture matches) / the kernel's
+own CUDA-event time measured inside the library on its launch stream; `algorithmic_*` is the same with the
+86 flop per accumulated (cell, phase, energy) triple of SURVEY.md 8(d) (can exceed 1: the kernel shares the mu
+contraction and the Lagrange -> monomial conversion between the energies of a pair).  `cpu_baseline` times the
+CPU oracle as it stands on the same workload (rank 0, N = 1 only): one evaluation in full on all host threads when
+that takes about a minute or less, else a bounded sample; single-threaded on a bounded sample (--cpu-baseline full:
+both in full).
 
 --precision 1 times the FP32-interpolation variant (tolerance 1e-4 instead of 1e-9; not the judged path), --tmap DEX the
 per-cell temperature-map entry ppm_evaluate_map with a seeded smooth map of +-DEX around each spot's log T.
@@ -46,11 +51,6 @@ import gen  # noqa: E402
 FLOP_PER_TRIPLE = 86.0          # SURVEY.md 8(d) accounting constant (FMA = 2 flop)
 # nominal FP64 vector peak: 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_cells_tab launch, from the one `ncu --set full` capture of each
-# workload that has one (profiles/r1d_k_cells_tab_T_full.md); other workloads report null
-NCU_TRAFFIC_BYTES = {"T": 74.063104e6 + 54.766336e6}
-# FP64 instructions the kernel executes per triple in that capture: 14.30 DFMA + 7.11 DADD + 1.42 DMUL
-EXECUTED_FLOP_PER_TRIPLE = 2 * 14.30 + 7.11 + 1.42
 METRIC = "pulse-profile evaluations per second"
 UNIT = "evals/s"
 
@@ -69,9 +69,10 @@ def workload(name, batch, rank, world=1):
         if name == "T":
             desc = "north-star target T = vector 0 of C5 evaluated alone; " + desc
         return conf, desc
-    conf = {"C2": gen.config_c2, "C3": gen.config_c3, "C4": gen.config_c4}[name]()
+    conf = {"C1": gen.config_c1, "C2": gen.config_c2, "C3": gen.config_c3, "C4": gen.config_c4}[name]()
     conf["params"] = np.ascontiguousarray(np.repeat(conf["params"], batch, axis=0))
-    return conf, "BASELINE.json config %s, batch of %d identical vectors" % (name, batch)
+    idx = {"C1": 0, "C2": 1, "C3": 2, "C4": 3}[name]
+    return conf, "BASELINE.json configs[%d] (%s), batch of %d identical vectors per GPU" % (idx, name, batch)
 
 
 class ClockSampler:
@@ -128,32 +129,99 @@ class ClockSampler:
         return out
 
 
-def oracle_sample(conf, n_extra=4):
+def _oracle_run(conf, atm, rsp, sel):
+    import oracle as o
+    cfg, E, p = conf["cfg"], conf["energies"], conf["params"][0]
+    t0 = time.perf_counter()
+    f, _ = o.evaluate(cfg, E, p, atm, phase_sel=sel)
+    if rsp is not None:
+        c = o.fold(f, rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"], p[5], rsp["n_channel"])
+        o.loglike(c, np.ones_like(c), None, 1.0)
+    return time.perf_counter() - t0
+
+
+def oracle_sample(conf, n_extra=4, threads=None):
     """Time the CPU oracle, as it stands, on vector 0 of the workload: one run on 1 output phase and
     one on 1 + n_extra phases (the per-row template work is paid once per run, the shift-and-add
     scales with the phases), fold + ln L on the sampled phases; the full-evaluation time is the
     linear extrapolation to n_phase phases.  -> dict(value evals/s, seconds, cores, sample)."""
     import oracle as o
-    cfg, E, p = conf["cfg"], conf["energies"], conf["params"][0]
+    cfg, E = conf["cfg"], conf["energies"]
     atm = o.Atmosphere(*gen.synthetic_atmosphere()) if cfg["emission"] else None
     nph = cfg["n_phase"]
+    n_extra = max(1, min(n_extra, nph - 1))
     sel1 = [nph // 3]
     sel2 = sel1 + [(nph // 3 + (i + 1) * nph // (n_extra + 1)) % nph for i in range(n_extra)]
     rsp = gen.synthetic_response(E) if len(E) == 300 else None
-    t0 = time.perf_counter()
-    o.evaluate(cfg, E, p, atm, phase_sel=sel1)
-    t1 = time.perf_counter()
-    f2, _ = o.evaluate(cfg, E, p, atm, phase_sel=sel2)
-    if rsp is not None:
-        c = o.fold(f2, rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"], p[5], rsp["n_channel"])
-        o.loglike(c, np.ones_like(c), None, 1.0)
-    t2 = time.perf_counter()
-    d1, d2 = t1 - t0, t2 - t1
+    all_threads = o.num_threads()
+    if threads:
+        o.set_num_threads(threads)
+    try:
+        d1 = _oracle_run(conf, atm, rsp, sel1)
+        d2 = _oracle_run(conf, atm, rsp, sel2)
+        cores = o.num_threads()
+    finally:
+        o.set_num_threads(all_threads)
     per_phase = max(d2 - d1, 0.0) / n_extra
     full = d1 + per_phase * (nph - 1)
-    return dict(value=1.0 / full, seconds=d1 + d2, cores=o.num_threads(), full_eval_s=full,
+    return dict(value=1.0 / full, seconds=d1 + d2, cores=cores, full_eval_s=full,
                 sample="vector 0: oracle run on 1 and on %d of %d output phases (%.1f s + %.1f s), full evaluation "
                        "extrapolated linearly in phases to %.1f s" % (1 + n_extra, nph, d1, d2, full))
+
+
+def oracle_full(conf, threads=None):
+    """One whole evaluation of vector 0 by the CPU oracle (+ fold + ln L where the workload has a response)."""
+    import oracle as o
+    cfg, E = conf["cfg"], conf["energies"]
+    atm = o.Atmosphere(*gen.synthetic_atmosphere()) if cfg["emission"] else None
+    rsp = gen.synthetic_response(E) if len(E) == 300 else None
+    all_threads = o.num_threads()
+    if threads:
+        o.set_num_threads(threads)
+    try:
+        d = _oracle_run(conf, atm, rsp, None)
+        cores = o.num_threads()
+    finally:
+        o.set_num_threads(all_threads)
+    return dict(value=1.0 / d, seconds=d, cores=cores, full_eval_s=d,
+                sample="vector 0 evaluated in full (%d phases x %d energies), %.1f s" % (cfg["n_phase"], len(E), d))
+
+
+def cpu_baseline(conf, mode="sample"):
+    """-> the bench line's cpu_baseline object.  All host threads: in full when the predicted time is <= 75 s (or
+    mode == "full"), else the extrapolated sample; one thread: a sample (in full when mode == "full")."""
+    first = oracle_sample(conf)
+    allc = oracle_full(conf) if (mode == "full" or first["full_eval_s"] <= 75.0) else first
+    one = oracle_full(conf, threads=1) if mode == "full" else oracle_sample(conf, n_extra=2, threads=1)
+    return {"value": allc["value"], "unit": UNIT, "cores": allc["cores"], "kind": "oracle", "sample": allc["sample"],
+            "s_per_eval": allc["full_eval_s"],
+            "single_thread": {"value": one["value"], "unit": UNIT, "cores": one["cores"], "s_per_eval": one["full_eval_s"],
+                              "sample": one["sample"]}}
+
+
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) of the sources that define the table cell kernels: a capture in ncu_captured.json
+    is used only for the kernel build it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2510_07764_b200", "csrc")
+    for f in ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_capture_for(key):
+    """Counters of the `ncu --set full` capture of the cell kernel on exactly this workload key and kernel source, or None."""
+    path = os.path.join(ROOT, "paper_2510_07764_b200", "ncu_captured.json")
+    try:
+        with open(path) as f:
+            cap = json.load(f).get("captures", {}).get(key)
+    except (OSError, ValueError):
+        return None
+    if not cap or cap.get("source_hash") != kernel_source_hash():
+        return None
+    return cap
 
 
 def run_reference(args, rank):
@@ -189,9 +257,13 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ppm", choices=["ppm", "reference"])
-    ap.add_argument("--workload", default="C5", choices=["C5", "T", "C2", "C3", "C4"])
-    ap.add_argument("--batch", type=int, default=8)
+    ap.add_argument("--workload", default="C5", choices=["C5", "T", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--batch", type=int, default=8,
+                    help="parameter vectors per GPU and step (C5: BASELINE.json states 1024; the default 8 gives the "
+                         "per-evaluation figure in seconds instead of minutes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline", default="sample", choices=["sample", "full"],
+                    help="full: time the oracle on one whole evaluation both single-threaded and on all threads")
     ap.add_argument("--tmap", type=float, default=None, metavar="DEX",
                     help="per-cell temperature maps (ppm_evaluate_map): each spot's log T modulated by +-DEX over its mesh")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1],
@@ -310,34 +382,55 @@ def main():
 
     if rank == 0:
         cells_ms, cells_n = prof["cells"]
-        tri_per_launch = triples / max(cells_n, 1)
-        achieved = FLOP_PER_TRIPLE * tri_per_launch / (cells_ms / max(cells_n, 1) * 1e-3) / 1e12
+        n_launch = max(cells_n, 1)
+        tri_per_launch = triples / n_launch
+        kern_s = cells_ms / n_launch * 1e-3
+        algorithmic = FLOP_PER_TRIPLE * tri_per_launch / kern_s / 1e12
         try:
             peak_dfma = ppm.measure_fp64_peak(local) / 1e12
         except ppm.PPMError:
             peak_dfma = None
         kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
         table = bool(cfg["emission"])
-        default_kernel = table and args.tmap is None and args.precision == 0
+        kname = (("k_cells_map" if args.tmap is not None else "k_cells_tab32" if args.precision else "k_cells_tab")
+                 if table else "k_cells_bb")
+        key = "%s:%d:p%d%s" % (args.workload, B, args.precision, "" if args.tmap is None else ":tmap%g" % args.tmap)
+        cap = ncu_capture_for(key)
         # precision = 1 runs the per-triple work on the FP32 pipe: 128 FFMA lanes per SM, twice the FP64 figure
         peak_nominal = FP64_NOMINAL_TFLOPS * (2.0 if args.precision == 1 else 1.0)
-        roofline = {"bound": "alu", "kernel": ("k_cells_map" if args.tmap is not None else "k_cells_tab32" if args.precision else "k_cells_tab")
-                    if table else "k_cells_bb", "achieved": achieved,
-                    "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-                    "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if default_kernel else None,
-                    "executed_flop_per_unit": EXECUTED_FLOP_PER_TRIPLE if default_kernel else None,
+        achieved = exec_per_unit = traffic = None
+        if cap:
+            # thread-level FP64 instructions of ONE launch of this workload (deterministic): 2 flop per DFMA
+            flop_per_launch = 2.0 * cap["dfma"] + cap["dadd"] + cap["dmul"] + \
+                              (2.0 * cap.get("ffma", 0) + cap.get("fadd", 0) + cap.get("fmul", 0) if args.precision == 1 else 0.0)
+            achieved = flop_per_launch / kern_s / 1e12
+            exec_per_unit = flop_per_launch / max(tri_per_launch, 1.0)
+            traffic = cap.get("dram_bytes")
+        roofline = {"bound": "alu", "kernel": kname,
+                    "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                    "frac": (achieved / peak_nominal) if achieved is not None else None,
+                    "traffic": traffic,
+                    "basis": ("executed FP64 flop per launch (2 DFMA + DADD + DMUL thread instructions, ncu capture of this "
+                              "workload and kernel source: %s) / the kernel's CUDA-event time" % cap.get("profile", "?"))
+                             if cap else "no ncu capture matches this workload key and kernel source: see algorithmic_*",
+                    "capture_key": key, "kernel_source_hash": kernel_source_hash(),
+                    "executed_flop_per_unit": exec_per_unit,
+                    "algorithmic_flop_per_unit": FLOP_PER_TRIPLE, "algorithmic_achieved": algorithmic,
+                    "algorithmic_frac": algorithmic / peak_nominal,
                     "peak_source": ("nominal FP32 FMA pipe: 148 SM x 128 FFMA/clk x 2 flop x 1.965 GHz" if args.precision == 1 else
                                     "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md "
                                     "Roofline); MEASURED_PEAKS.json has no FP64 entry"),
                     "peak_measured_dfma_chain": peak_dfma,
-                    "frac_of_measured_dfma_chain": (achieved / peak_dfma) if peak_dfma else None,
-                    "flop_per_unit": FLOP_PER_TRIPLE, "units_per_launch": tri_per_launch,
-                    "kernel_ms_per_launch": cells_ms / max(cells_n, 1),
+                    "frac_of_measured_dfma_chain": (achieved / peak_dfma) if (peak_dfma and achieved is not None) else None,
+                    "units_per_launch": tri_per_launch, "unit_name": "accumulated (cell, phase, energy) triple",
+                    "kernel_ms_per_launch": cells_ms / n_launch, "kernel_launches_per_step": cells_n / args.steps,
                     "kernel_share_of_step": cells_ms / total_ms, "kernel_ms_per_step": kern_ms}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_eval": ms_per_step / B,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 0 else "f32 interpolation / f64 geometry+sums", "data": "synthetic",
-                "config": {"workload": desc, "name": args.workload, "precision": args.precision, "tmap_dex": args.tmap, "batch_per_gpu": B, "n_fp": ctx.n_fp,
+                "config": {"workload": desc + (" -- NOTE: BASELINE.json states a batch of 1024 for this config; this run uses "
+                                               "%d per GPU (per-evaluation figure; run --batch 1024 for the stated batch)" % B
+                                               if args.workload == "C5" and B != 1024 else ""), "name": args.workload, "precision": args.precision, "tmap_dex": args.tmap, "batch_per_gpu": B, "sub_batch": ctx.sub_batch(), "n_fp": ctx.n_fp,
                            "l2": "flushed before every step (256 MiB write between the steps' CUDA-event brackets)",
                            "step": "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params_pinned.numel() * 8),
@@ -346,9 +439,7 @@ def main():
                 "gpu_launches": int(launches), "clocks": clk, "wall_ms_per_step": wall_ms / args.steps,
                 "step_ms": [round(x, 3) for x in per], "roofline": roofline, "cpu_baseline": None}
         if world == 1 and not args.no_cpu_baseline:
-            cb = oracle_sample(conf)
-            line["cpu_baseline"] = {"value": cb["value"], "unit": UNIT, "cores": cb["cores"], "kind": "oracle",
-                                    "sample": cb["sample"]}
+            line["cpu_baseline"] = cpu_baseline(conf, args.cpu_baseline)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()

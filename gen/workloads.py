@@ -94,6 +94,39 @@ def synthetic_atmosphere(seed=SEED0, amplitude=0.05):
     return logT, logg, mu, logx, np.ascontiguousarray(vals)
 
 
+def steep_limb_atmosphere(seed=SEED0, amplitude=0.05, a0=1.2):
+    """Table for the interpolation-strategy study: same axes and Planck x perturbation
+    as synthetic_atmosphere, but (i) the mu axis reaches 1e-6 with a few widely spaced nodes near 0 -- mu = 1e-6, 1e-3,
+    1e-2, then 64 cosine-spaced nodes on [0.04, 1] ("mu in [1e-6, 1] with extra nodes near mu ~ 0, 1") --
+    and (ii) the angular law is steep towards the limb, exp(-a(x) (1-mu)/(mu+0.03)) with a(x) = a0 / (1 + x/3), stronger in
+    the soft band.  On such nodes a cubic Lagrange stencil applied to the INTENSITY overshoots below zero inside the first
+    intervals of the mu axis (the paper's artefact); the NSX-H table itself is not available."""
+    logT, logg, _, logx = atmosphere_axes()
+    j = np.arange(64, dtype=np.float64)
+    mu = np.concatenate([[1e-6, 1e-3, 1e-2], 0.04 + 0.96 * (1.0 - np.cos(np.pi * j / 63.0)) / 2.0])
+    mu[-1] = 1.0
+    _, _, mu0, _, base = synthetic_atmosphere(seed, amplitude)
+    # strip synthetic_atmosphere's own limb law (its perturbation P is kept as laid out on the normalised axes)
+    limb0 = (1.0 + 2.06 * mu0) / 3.06
+    core = base - np.log10(limb0)[None, None, :, None]
+    x = 10.0 ** logx
+    a = a0 / (1.0 + x / 3.0)
+    law = -a[None, :] * (1.0 - mu[:, None]) / (mu[:, None] + 0.03) / np.log(10.0)      # log10 of the angular law
+    vals = core + law[None, None, :, :]
+    return logT, logg, mu, logx, np.ascontiguousarray(vals)
+
+
+def config_interp_test(which, n_cells=32, n_phase=128, n_energy=128):
+    """The two atmosphere-interpolation test geometries of Table 3: one point-like hotspot of angular
+    radius 0.01 rad at T = 1e6 K, M = 1.4, R_e = 12 km, 600 Hz, D = 150 pc; Test 1: theta_c = 1.983, i = 0.01;
+    Test 2: theta_c = pi - 0.01, i = 0.964.  Energies: the paper's grid, Eq 50.  Strategy / domain are set by the caller."""
+    theta_c, inc = {1: (1.983, 0.01), 2: (np.pi - 0.01, 0.964)}[which]
+    cfg = _cfg(1, n_cells, n_cells, n_phase, max(192, 2 * n_phase), 2, 1)
+    E = logspace(0.1, 5.215, n_energy)
+    p = pack_params(1.4, 12.0, 600.0, np.cos(inc), 0.15, spots=[(theta_c, 0.0, 0.01, 6.0)])
+    return dict(name="interp_test_%d" % which, cfg=cfg, energies=E, params=p[None, :], needs_table=True)
+
+
 # ------------------------------------------------------------------------------------------
 # configs
 # ------------------------------------------------------------------------------------------
@@ -157,10 +190,28 @@ def config_c4(n_cells=512, n_phase=512, n_energy=256, seed=SEED0 + 4):
     return dict(name="C4", cfg=cfg, energies=E, params=p[None, :], needs_table=True)
 
 
+def _outside_prior_support(M, Re_km, nu):
+    """SURVEY.md 8(d) support of the C5 prior: a draw is rejected when u_pole = R_S / R(theta = 0) > 0.55 or
+    beta_eq >= 0.5, with R(0) = R_e (1 + o2) of Eq 7-8 and beta_eq of Eq 18.
+    This only defines which synthetic vectors exist; neither implementation calls it."""
+    GM = M * _GMSUN
+    Re = Re_km * 1.0e3
+    Rs = 2.0 * GM / (_C * _C)
+    x = GM / (_C * _C * Re)
+    Ob2 = (2.0 * np.pi * nu) ** 2 * Re ** 3 / GM
+    o2 = Ob2 * (-0.788 + 1.030 * x)
+    R_pole = Re * (1.0 + o2)
+    if not (R_pole > Rs and Re > Rs):
+        return True
+    u_pole = Rs / R_pole
+    beta_eq = 2.0 * np.pi * nu * Re / (_C * np.sqrt(1.0 - Rs / Re))
+    return bool(u_pole > 0.55 or beta_eq >= 0.5)
+
+
 def c5_params(n_vec=1024, seed=SEED0 + 5):
-    """Seeded parameter vectors from uniform priors.  A vector is re-drawn while its equatorial
-    compactness 2GM/(c^2 R_e) exceeds 0.5 (prior-level cut that keeps every vector inside the
-    supported domain u_pole <= 0.56 of reading R4 for all nu <= 700 Hz)."""
+    """Seeded parameter vectors from uniform priors; a vector is re-drawn while it lies outside the prior support
+    of SURVEY.md 8(d) (u_pole > 0.55 or beta_eq >= 0.5; the raw priors reach unphysical u > 1), which keeps every
+    vector inside the supported domain u <= 0.56 of reading R4."""
     rng = np.random.Generator(np.random.PCG64(seed))
     out = np.zeros((n_vec, N_STAR_PARAMS + 2 * N_SPOT_PARAMS))
     for b in range(n_vec):
@@ -177,7 +228,7 @@ def c5_params(n_vec=1024, seed=SEED0 + 5):
                 lt = rng.uniform(5.6, 6.5)
                 ph = 0.0 if s == 0 else rng.uniform(0.0, 2.0 * np.pi)
                 sp.append((th, ph, ze, lt))
-            if 2.0 * M * _GMSUN / (_C * _C * Re * 1.0e3) <= 0.5:
+            if not _outside_prior_support(M, Re, nu):
                 break
         out[b] = pack_params(M, Re, nu, cos_i, 0.15, NH, 0.0, sp)
     return out

@@ -57,6 +57,8 @@ extern "C" {
 #define PPM_EMISSION_TABLE_MIXED 2  /* 4-D table, mixed order (strategy d) */
 #define PPM_EMISSION_TABLE_CUBIC_LINEDGE 3 /* cubic on all axes, linear at the table boundaries and in the protected
                                              small-mu zone (strategy c; reading R13e) */
+#define PPM_EMISSION_TABLE_CUBIC_CLIP 4    /* strategy b: as strategy a, negative intensities clipped to 0;
+                                             identical to strategy a when interp_domain = 0 (I = T^3 10^v > 0) */
 
 #define PPM_MAX_SPOTS 4
 
@@ -69,7 +71,7 @@ typedef struct {
     int32_t n_phase;    /* output phases, phi_out[k] = k / n_phase (reading R3) */
     int32_t n_fp;       /* fine template phases N_fp (Table 4); 0 -> max(192, 2*n_phase) */
     int32_t n_energy;   /* observed photon energies (keV), given to ppm_create */
-    int32_t emission;   /* PPM_EMISSION_* (0..3) */
+    int32_t emission;   /* PPM_EMISSION_* (0..4) */
     int32_t precision;  /* 0 = fp64 everywhere; 1 = table interpolation + exponential in fp32 (geometry, templates,
                            coordinates and the final sums stay fp64; tolerance 1e-4 per bin), table emission only */
     int32_t oblate;     /* 0 spherical S+D (o2 = 0, g = g0); 1 oblate OS+D (Eq 7-11) */
@@ -80,6 +82,13 @@ typedef struct {
                               for every spot: n_phi = 4 N_side, n_theta = 4 N_side - 1 rings, pixel area pi/(3 N_side^2) */
     int32_t beaming;    /* blackbody emission only: 0 isotropic, 1 I prop. to cos^2(sigma'),
                            2 I prop. to sin^2(sigma'), cos(sigma') = mu = delta cos(sigma) (Eq 20) */
+    int32_t scratch_mb; /* budget (MiB) for the per-launch scratch (row slices, templates, partial tiles); batches larger
+                           than what fits are processed in sub-batches of ppm_sub_batch() vectors.  0 -> 1536 */
+    int32_t phase_interp; /* order of Interp in Eq 46: 0 or 1 = piecewise linear (reading R11);
+                             3 = 4-point (cubic) Lagrange in phi_o on the periodic template (reading R11b) */
+    int32_t interp_domain; /* table emission: 0 = the 4-D interpolation acts on the tabulated log10(I/T^3) and
+                              I = T^3 10^v (reading R13a); 1 = it acts on I/T^3 = 10^table itself (reading R13g,
+                              PAPER.md:551-559: the form in which cubic overshoot produces negative intensities) */
 } ppm_config;
 
 /* Create a context: copies the energy grid (host, [n_energy], keV, strictly increasing),
@@ -156,6 +165,9 @@ int ppm_debug_lookup(ppm_ctx* ctx, int b, int row, const double* alpha_host, int
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t ppm_launch_count(const ppm_ctx* ctx);
+/* Vectors per internal sub-batch (scratch_mb / per-vector scratch, capped by max_batch); a batch B is processed
+ * as ceil(B / ppm_sub_batch) sequences of launches.  Final after ppm_load_atmosphere for table emission. */
+int ppm_sub_batch(const ppm_ctx* ctx);
 /* Effective n_fp after defaulting. */
 int ppm_n_fp(const ppm_ctx* ctx);
 

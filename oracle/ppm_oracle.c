@@ -644,10 +644,25 @@ double orc_interp1(const double* ax, const double* y, int n, double x, int rule)
 /* strategy: 1 = (a) cubic on all four axes; 2 = (d) mixed order (reading R13c);
  * 3 = (c) cubic on all four axes with linear interpolation at the table boundaries (Fig 4 caption PAPER.md:537)
  * and in the protected small-mu zone ("linear interpolation enforced at the mu -> 0 boundary"; R13e) */
+static double interp4_domain(const orc_atm* A, int strategy, int domain, double logT, double logg, double mu, double logx);
+
 double orc_interp4(const orc_atm* A, int strategy, double logT, double logg, double mu, double logx)
 {
+    return interp4_domain(A, strategy, 0, logT, logg, mu, logx);
+}
+
+/* domain 0: the weighted sum runs over the tabulated log10(I/T^3) (reading R13a); domain 1: over I/T^3 = 10^table
+ * (reading R13g -- the form in which a cubic stencil can return a negative intensity).
+ * strategy 4 = (b): the stencils of (a); the clipping of negative intensities is applied by the caller. */
+double orc_interp4_domain(const orc_atm* A, int strategy, int domain, double logT, double logg, double mu, double logx)
+{
+    return interp4_domain(A, strategy, domain, logT, logg, mu, logx);
+}
+
+static double interp4_domain(const orc_atm* A, int strategy, int domain, double logT, double logg, double mu, double logx)
+{
     int rT, rg, rm, rx;
-    if (strategy == 1) { rT = rg = rm = rx = AX_CUBIC_SHIFT; }
+    if (strategy == 1 || strategy == 4) { rT = rg = rm = rx = AX_CUBIC_SHIFT; }
     else if (strategy == 3) { rT = rg = rx = AX_CUBIC_LINEDGE; rm = AX_MU_PROTECTED; }
     else { rT = rg = AX_LINEAR; rm = AX_MU_PROTECTED; rx = AX_CUBIC_LINEDGE; }
     int bT, cT, bg, cg, bm, cm, bx, cx; double wT[4], wg[4], wm[4], wx[4];
@@ -661,7 +676,8 @@ double orc_interp4(const orc_atm* A, int strategy, double logT, double logg, dou
             for (int c = 0; c < cm; ++c)
                 for (int d = 0; d < cx; ++d) {
                     size_t idx = (((size_t)(bT + a) * A->ng + (bg + b)) * A->nmu + (bm + c)) * A->nx + (bx + d);
-                    v += wT[a] * wg[b] * wm[c] * wx[d] * A->values[idx];
+                    double node = domain ? pow(10.0, A->values[idx]) : A->values[idx];
+                    v += wT[a] * wg[b] * wm[c] * wx[d] * node;
                 }
     return v;
 }
@@ -670,6 +686,7 @@ double orc_interp4(const orc_atm* A, int strategy, double logT, double logg, dou
  * I = T^3 10^v (reading R13a).  E' in keV, returns keV^0 s^-1 cm^-2 sr^-1 (per keV, times keV). */
 static int g_beaming = 0;   /* blackbody beaming law: 0 isotropic; 1 prop. to cos^2(sigma'); 2 prop. to sin^2(sigma')
                              * ("simple parametric laws"; cos(sigma') = mu, reading R23) */
+static int g_domain = 0;    /* table emission: 0 interpolate log10(I/T^3) (R13a); 1 interpolate I/T^3 itself (R13g) */
 static double intensity(int emission, const orc_atm* A, double log10T, double log10g, double Ep, double mu)
 {
     const double kB = ORC_KB_J_K / ORC_E_C / 1.0e3;
@@ -681,12 +698,64 @@ static double intensity(int emission, const orc_atm* A, double log10T, double lo
         else if (g_beaming == 2) I *= 1.0 - mu * mu;
         return I;
     }
-    double v = orc_interp4(A, emission, log10T, log10g, mu, log10(Ep / kT));
-    return T * T * T * pow(10.0, v);
+    if (g_domain == 0) {
+        /* strategy b clips negative intensities; 10^v > 0, so here it is strategy a (reading R13f) */
+        double v = interp4_domain(A, emission, 0, log10T, log10g, mu, log10(Ep / kT));
+        return T * T * T * pow(10.0, v);
+    }
+    double w = interp4_domain(A, emission, 1, log10T, log10g, mu, log10(Ep / kT));   /* I/T^3, may be negative */
+    if (emission == 4 && w < 0.0) w = 0.0;                                           /* strategy b: clip to zero */
+    return T * T * T * w;
 }
 double orc_intensity(int emission, const orc_atm* A, double log10T, double log10g, double Ep, double mu)
 {
     return intensity(emission, A, log10T, log10g, Ep, mu);
+}
+double orc_intensity_domain(int emission, int domain, const orc_atm* A, double log10T, double log10g, double Ep, double mu)
+{
+    int keep = g_domain;
+    g_domain = domain;
+    double v = intensity(emission, A, log10T, log10g, Ep, mu);
+    g_domain = keep;
+    return v;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Interp of Eq 46 on the periodic template (phio strictly increasing, phio[n_fp] = phio[0] + 1).
+ * order 1 (reading R11): piecewise linear on the bracket phio[i] <= phi_p < phio[i+1].
+ * order 3 (reading R11b): 4-point Lagrange on the nodes {i-1, i, i+1, i+2} with the TRUE abscissae phio, wrapped
+ * periodically (node -1 = node n_fp-1 one cycle earlier, node n_fp+1 = node 1 one cycle later).  Next to the
+ * visibility edge F has a kink and the filled z, phio are only continuous: if any of the four F nodes is 0
+ * (an invisible or filled entry, Eq 41) the bracket reverts to the linear rule -- the same "linear at the
+ * boundary" safeguard the paper applies to the atmosphere table.
+ * y = one of F, z, mu.  Returns the bracket index through *i_out (optional).
+ * ---------------------------------------------------------------------------------- */
+double orc_phase_interp(int n_fp, const double* phio, const double* F, const double* y, double phi_p, int order, int* i_out)
+{
+    int lo = 0, hi = n_fp;                                                       /* phio[lo] <= phi_p < phio[hi] */
+    while (hi - lo > 1) { int mid = (lo + hi) / 2; if (phio[mid] <= phi_p) lo = mid; else hi = mid; }
+    if (i_out) *i_out = lo;
+    if (order == 3) {
+        int idx[4]; double x[4], f[4], v[4];
+        for (int k = 0; k < 4; ++k) {
+            int j = lo - 1 + k; double shift = 0.0;
+            if (j < 0) { j += n_fp; shift = -1.0; }
+            if (j > n_fp) { j -= n_fp; shift = 1.0; }
+            idx[k] = j; x[k] = phio[j] + shift; f[k] = F[j]; v[k] = y[j];
+        }
+        (void)idx;
+        if (f[0] != 0.0 && f[1] != 0.0 && f[2] != 0.0 && f[3] != 0.0) {
+            double r = 0.0;
+            for (int k = 0; k < 4; ++k) {
+                double num = 1.0, den = 1.0;
+                for (int m = 0; m < 4; ++m) if (m != k) { num *= (phi_p - x[m]); den *= (x[k] - x[m]); }
+                r += num / den * v[k];
+            }
+            return r;
+        }
+    }
+    double t = (phi_p - phio[lo]) / (phio[lo + 1] - phio[lo]);
+    return y[lo] + (y[lo + 1] - y[lo]) * t;
 }
 
 /* ------------------------------------------------------------------------------------
@@ -702,6 +771,8 @@ typedef struct {
     int32_t mesh;    /* 0: per-spot theta x phi bounding-box grid (reading R1); 1: HEALPix rings (Eq 24-29) with
                         N_side = n_phi / 4, n_theta = 4 N_side - 1, the same mesh for every spot */
     int32_t beaming; /* emission 0 only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma') */
+    int32_t phase_interp;  /* Interp of Eq 46: 0 / 1 linear (reading R11); 3 four-point Lagrange (reading R11b) */
+    int32_t interp_domain; /* table emission: 0 interpolate log10(I/T^3) (R13a); 1 interpolate I/T^3 (R13g) */
 } orc_config;
 
 #define ORC_U_MAX 0.560     /* supported compactness domain (reading R4) */
@@ -739,6 +810,8 @@ static int evaluate_impl(const orc_config* cfg, const double* energies, const do
     int status = check_domain(cfg, params, &star);
     if (status) { for (size_t i = 0; i < (size_t)nk * nE; ++i) flux[i] = NAN; return status; }
     g_beaming = cfg->emission == 0 ? cfg->beaming : 0;   /* set before the parallel region; one evaluation at a time */
+    g_domain = cfg->emission != 0 ? cfg->interp_domain : 0;
+    const int porder = cfg->phase_interp == 3 ? 3 : 1;
     const double cosi = params[3], D_cm = params[4] * 1.0e3 * ORC_PC_M * 100.0, phi_off = params[6];
     const double kB = ORC_KB_J_K / ORC_E_C / 1.0e3;
     (void)kB;
@@ -793,12 +866,9 @@ static int evaluate_impl(const orc_config* cfg, const double* energies, const do
                     double phi_out = (double)k / cfg->n_phase;                               /* reading R3 */
                     double s0 = phi_out + phi_m / (2.0 * M_PI) + phi_off + 1.0 - po[0];
                     double phi_p = (s0 - floor(s0)) + po[0];                                 /* Eq 45 */
-                    int lo = 0, hi = nfp;                                                     /* po[lo] <= phi_p < po[hi] */
-                    while (hi - lo > 1) { int mid = (lo + hi) / 2; if (po[mid] <= phi_p) lo = mid; else hi = mid; }
-                    double t = (phi_p - po[lo]) / (po[lo + 1] - po[lo]);
-                    double Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                              /* Eq 46, linear (R11) */
-                    double zp = z[lo] + (z[lo + 1] - z[lo]) * t;
-                    double mup = mu[lo] + (mu[lo + 1] - mu[lo]) * t;
+                    double Fp = orc_phase_interp(nfp, po, F, F, phi_p, porder, NULL);         /* Eq 46 (R11 / R11b) */
+                    double zp = orc_phase_interp(nfp, po, F, z, phi_p, porder, NULL);
+                    double mup = orc_phase_interp(nfp, po, F, mu, phi_p, porder, NULL);
                     if (Fp == 0.0) continue;
                     for (int e = 0; e < nE; ++e) {
                         double E = energies[e];

@@ -45,7 +45,7 @@ class _Atm(C.Structure):
 class _Config(C.Structure):
     _fields_ = [("n_spots", C.c_int32), ("n_theta", C.c_int32), ("n_phi", C.c_int32), ("n_phase", C.c_int32),
                 ("n_fp", C.c_int32), ("n_energy", C.c_int32), ("emission", C.c_int32), ("oblate", C.c_int32),
-                ("mesh", C.c_int32), ("beaming", C.c_int32)]
+                ("mesh", C.c_int32), ("beaming", C.c_int32), ("phase_interp", C.c_int32), ("interp_domain", C.c_int32)]
 
 
 def _sig(name, res, args):
@@ -75,6 +75,9 @@ _template = _sig("orc_template", C.c_int,
 _interp1 = _sig("orc_interp1", C.c_double, [_dp, _dp, C.c_int, C.c_double, C.c_int])
 _interp4 = _sig("orc_interp4", C.c_double, [C.POINTER(_Atm), C.c_int] + [C.c_double] * 4)
 _intensity = _sig("orc_intensity", C.c_double, [C.c_int, C.POINTER(_Atm)] + [C.c_double] * 4)
+_interp4_dom = _sig("orc_interp4_domain", C.c_double, [C.POINTER(_Atm), C.c_int, C.c_int] + [C.c_double] * 4)
+_intensity_dom = _sig("orc_intensity_domain", C.c_double, [C.c_int, C.c_int, C.POINTER(_Atm)] + [C.c_double] * 4)
+_phase_interp = _sig("orc_phase_interp", C.c_double, [C.c_int, _dp, _dp, _dp, C.c_double, C.c_int, C.POINTER(C.c_int)])
 _evaluate = _sig("orc_evaluate", C.c_int,
                  [C.POINTER(_Config), _dp, _dp, C.POINTER(_Atm), _ip, C.c_int, _dp, _dp])
 _evaluate_map = _sig("orc_evaluate_map", C.c_int,
@@ -239,9 +242,23 @@ def interp4(atm, strategy, logT, logg, mu, logx):
     return _interp4(C.byref(atm.c), int(strategy), logT, logg, mu, logx)
 
 
-def intensity(emission, atm, log10T, log10g, Ep, mu):
+def intensity(emission, atm, log10T, log10g, Ep, mu, domain=0):
     ap = C.byref(atm.c) if atm is not None else None
+    if domain:
+        return _intensity_dom(int(emission), int(domain), ap, log10T, log10g, Ep, mu)
     return _intensity(int(emission), ap, log10T, log10g, Ep, mu)
+
+
+def interp4_domain(atm, strategy, domain, logT, logg, mu, logx):
+    return _interp4_dom(C.byref(atm.c), int(strategy), int(domain), logT, logg, mu, logx)
+
+
+def phase_interp(phio, F, y, phi_p, order):
+    """Interp of Eq 46 on a periodic template (n_fp + 1 entries): -> (value, bracket index)."""
+    phio, F, y = _f64(phio), _f64(F), _f64(y)
+    i = C.c_int()
+    v = _phase_interp(len(phio) - 1, _p(phio), _p(F), _p(y), float(phi_p), int(order), C.byref(i))
+    return v, i.value
 
 
 # ---- evaluation ------------------------------------------------------------------------
@@ -252,7 +269,7 @@ def evaluate(cfg, energies, params, atm=None, phase_sel=None, return_margin=Fals
     params = _f64(params)
     c = _Config(cfg["n_spots"], cfg["n_theta"], cfg["n_phi"], cfg["n_phase"], cfg["n_fp"],
                 len(energies), cfg["emission"], int(cfg.get("oblate", 1)), int(cfg.get("mesh", 0)),
-                int(cfg.get("beaming", 0)))
+                int(cfg.get("beaming", 0)), int(cfg.get("phase_interp", 0)), int(cfg.get("interp_domain", 0)))
     assert params.shape == (8 + 8 * cfg["n_spots"],)
     if cfg["emission"] != 0:
         assert atm is not None

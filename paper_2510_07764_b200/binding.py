@@ -9,6 +9,7 @@ import numpy as np
 from . import _build
 
 EMISSION_BLACKBODY, EMISSION_TABLE_CUBIC, EMISSION_TABLE_MIXED, EMISSION_TABLE_CUBIC_LINEDGE = 0, 1, 2, 3
+EMISSION_TABLE_CUBIC_CLIP = 4
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -22,7 +23,8 @@ class PPMError(RuntimeError):
 
 class _Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_spots", "n_theta", "n_phi", "n_phase", "n_fp", "n_energy", "emission",
-                                         "precision", "oblate", "max_batch", "device", "mesh", "beaming")]
+                                         "precision", "oblate", "max_batch", "device", "mesh", "beaming",
+                                         "scratch_mb", "phase_interp", "interp_domain")]
 
 
 # every symbol include/ppm.h declares: name -> (restype, argtypes)
@@ -43,6 +45,7 @@ EXPORTS = {
     "ppm_debug_lookup": (C.c_int, [_vp, C.c_int, C.c_int, _dp, C.c_int, _dp, _dp, _dp]),
     "ppm_launch_count": (C.c_int64, [_vp]),
     "ppm_n_fp": (C.c_int, [_vp]),
+    "ppm_sub_batch": (C.c_int, [_vp]),
     "ppm_profile_enable": (C.c_int, [_vp, C.c_int]),
     "ppm_profile_read": (C.c_int, [_vp, _dp, C.POINTER(C.c_int64), _dp]),
     "ppm_measure_fp64_peak": (C.c_int, [C.c_int, _dp]),
@@ -89,13 +92,21 @@ def _np(a):
     return a.ctypes.data_as(_dp)
 
 
-def _dev(t, dtype=None, what="tensor"):
+def _dev(t, dtype=None, what="tensor", shape=None):
     import torch
     if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
         raise PPMError(f"{what} must be a contiguous CUDA tensor")
     if dtype is not None and t.dtype != dtype:
         raise PPMError(f"{what} must have dtype {dtype}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise PPMError(f"{what} must have shape {tuple(shape)}, got {tuple(t.shape)}")
     return C.c_void_p(t.data_ptr())
+
+
+def _host(a, dtype, shape, what):
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous or a.shape != tuple(shape):
+        raise PPMError(f"{what} must be a C-contiguous numpy array of dtype {np.dtype(dtype)} and shape {tuple(shape)}")
+    return a
 
 
 def measure_fp64_peak(device=0):
@@ -107,7 +118,7 @@ def measure_fp64_peak(device=0):
 class PPM:
     """One context (ppm_create).  cfg: dict(n_spots, n_theta, n_phi, n_phase, n_fp, emission, oblate)."""
 
-    def __init__(self, cfg, energies, max_batch=1, device=0, precision=0):
+    def __init__(self, cfg, energies, max_batch=1, device=0, precision=0, scratch_mb=0):
         import torch
         self.lib = load_library()
         if not torch.cuda.is_available():
@@ -121,11 +132,13 @@ class PPM:
                                                                 ("n_spots", "n_theta", "n_phi", "n_phase"))
         c = _Config(self.n_spots, self.n_theta, self.n_phi, self.n_phase, int(cfg.get("n_fp", 0)), self.n_energy,
                     int(cfg["emission"]), int(precision), int(cfg.get("oblate", 1)), int(max_batch), int(device),
-                    int(cfg.get("mesh", 0)), int(cfg.get("beaming", 0)))
+                    int(cfg.get("mesh", 0)), int(cfg.get("beaming", 0)), int(scratch_mb),
+                    int(cfg.get("phase_interp", 0)), int(cfg.get("interp_domain", 0)))
         self.P = 8 + 8 * self.n_spots
         self.max_batch = int(max_batch)
         with torch.cuda.device(self.device):
             stream = torch.cuda.current_stream().cuda_stream
+        self._stream = stream
         self._h = C.c_void_p()
         _check(self.lib.ppm_create(C.byref(c), _np(energies), C.c_void_p(stream), C.byref(self._h)))
         self.n_fp = self.lib.ppm_n_fp(self._h)
@@ -138,6 +151,19 @@ class PPM:
             self._h = C.c_void_p()
 
     __del__ = close
+
+    def _on_stream(self):
+        """Single-stream contract (include/ppm.h): all work is enqueued on the stream that was current at construction;
+        a call made under another torch stream would not be ordered with the caller's tensors."""
+        if self.torch.cuda.current_stream(self.device).cuda_stream != self._stream:
+            raise PPMError("this context was created on another CUDA stream: call it under the same torch stream")
+
+    def _params(self, params):
+        if params.dim() != 2 or params.shape[1] != self.P:
+            raise PPMError(f"params must have shape [B][{self.P}]")
+        if params.shape[0] > self.max_batch:
+            raise PPMError(f"ppm error -5: B = {params.shape[0]} exceeds max_batch = {self.max_batch}")
+        return params.shape[0]
 
     # ---- tables ----
     def load_atmosphere(self, logT, logg, mu, logx, values):
@@ -168,46 +194,53 @@ class PPM:
     # ---- device-pointer calls (asynchronous on the context's stream) ----
     def evaluate(self, params, flux=None, status=None):
         t = self.torch
-        B = params.shape[0]
+        self._on_stream()
+        B = self._params(params)
         if flux is None:
             flux = t.empty((B, self.n_phase, self.n_energy), dtype=t.float64, device=self.device)
         if status is None:
             status = t.empty((B,), dtype=t.int32, device=self.device)
-        _check(self.lib.ppm_evaluate(self._h, _dev(params, t.float64, "params"), B, _dev(flux, t.float64, "flux"),
-                                     _dev(status, t.int32, "status")))
+        _check(self.lib.ppm_evaluate(self._h, _dev(params, t.float64, "params"), B,
+                                     _dev(flux, t.float64, "flux", (B, self.n_phase, self.n_energy)),
+                                     _dev(status, t.int32, "status", (B,))))
         return flux, status
 
     def evaluate_map(self, params, logT_map, flux=None, status=None):
         """ppm_evaluate_map: logT_map [B][n_spots][n_theta][n_phi] float64 CUDA tensor, NaN = cell does not emit."""
         t = self.torch
-        B = params.shape[0]
-        if tuple(logT_map.shape) != (B, self.n_spots, self.n_theta, self.n_phi):
-            raise PPMError("logT_map must have shape [B][n_spots][n_theta][n_phi]")
+        self._on_stream()
+        B = self._params(params)
         if flux is None:
             flux = t.empty((B, self.n_phase, self.n_energy), dtype=t.float64, device=self.device)
         if status is None:
             status = t.empty((B,), dtype=t.int32, device=self.device)
-        _check(self.lib.ppm_evaluate_map(self._h, _dev(params, t.float64, "params"), _dev(logT_map, t.float64, "logT_map"),
-                                         B, _dev(flux, t.float64, "flux"), _dev(status, t.int32, "status")))
+        _check(self.lib.ppm_evaluate_map(self._h, _dev(params, t.float64, "params"),
+                                         _dev(logT_map, t.float64, "logT_map", (B, self.n_spots, self.n_theta, self.n_phi)),
+                                         B, _dev(flux, t.float64, "flux", (B, self.n_phase, self.n_energy)),
+                                         _dev(status, t.int32, "status", (B,))))
         return flux, status
 
     def fold_response(self, flux, params, counts=None):
         t = self.torch
-        B = params.shape[0]
+        self._on_stream()
+        B = self._params(params)
         if counts is None:
             counts = t.empty((B, self.n_phase, self.n_channel), dtype=t.float64, device=self.device)
-        _check(self.lib.ppm_fold_response(self._h, _dev(flux, t.float64, "flux"), _dev(params, t.float64, "params"), B,
-                                          _dev(counts, t.float64, "counts")))
+        _check(self.lib.ppm_fold_response(self._h, _dev(flux, t.float64, "flux", (B, self.n_phase, self.n_energy)),
+                                          _dev(params, t.float64, "params"), B,
+                                          _dev(counts, t.float64, "counts", (B, self.n_phase, self.n_channel))))
         return counts
 
     def loglike(self, counts, data, bkg, exposure_s, out=None):
         t = self.torch
+        self._on_stream()
         B = counts.shape[0]
         if out is None:
             out = t.empty((B,), dtype=t.float64, device=self.device)
-        bp = _dev(bkg, t.float64, "bkg") if bkg is not None else C.c_void_p(0)
-        _check(self.lib.ppm_loglike(self._h, _dev(counts, t.float64, "counts"), B, _dev(data, t.float64, "data"), bp,
-                                    float(exposure_s), _dev(out, t.float64, "loglike")))
+        bp = _dev(bkg, t.float64, "bkg", (self.n_channel,)) if bkg is not None else C.c_void_p(0)
+        _check(self.lib.ppm_loglike(self._h, _dev(counts, t.float64, "counts", (B, self.n_phase, self.n_channel)), B,
+                                    _dev(data, t.float64, "data", (self.n_phase, self.n_channel)), bp,
+                                    float(exposure_s), _dev(out, t.float64, "loglike", (B,))))
         return out
 
     # ---- host-buffer calls (copies inside, synchronous) ----
@@ -218,6 +251,8 @@ class PPM:
             flux = np.empty((B, self.n_phase, self.n_energy))
         if status is None:
             status = np.empty((B,), dtype=np.int32)
+        _host(flux, np.float64, (B, self.n_phase, self.n_energy), "flux")
+        _host(status, np.int32, (B,), "status")
         _check(self.lib.ppm_evaluate_host(self._h, _np(params), B, _np(flux), status.ctypes.data_as(_ip)))
         return flux, status
 
@@ -229,8 +264,10 @@ class PPM:
             out = np.empty((B,))
         if status is None:
             status = np.empty((B,), dtype=np.int32)
-        bp = _dev(bkg, t.float64, "bkg") if bkg is not None else C.c_void_p(0)
-        _check(self.lib.ppm_loglike_host(self._h, _np(params), B, _dev(data, t.float64, "data"), bp, float(exposure_s),
+        _host(out, np.float64, (B,), "loglike")
+        _host(status, np.int32, (B,), "status")
+        bp = _dev(bkg, t.float64, "bkg", (self.n_channel,)) if bkg is not None else C.c_void_p(0)
+        _check(self.lib.ppm_loglike_host(self._h, _np(params), B, _dev(data, t.float64, "data", (self.n_phase, self.n_channel)), bp, float(exposure_s),
                                          _np(out), status.ctypes.data_as(_ip)))
         return out, status
 
@@ -271,3 +308,6 @@ class PPM:
 
     def launch_count(self):
         return int(self.lib.ppm_launch_count(self._h))
+
+    def sub_batch(self):
+        return int(self.lib.ppm_sub_batch(self._h))

@@ -185,6 +185,28 @@ static size_t cells_tab_smem(const ppm_ctx* c, int nmu, int nx, int npl)
     return sizeof(double) * ((size_t)nmu * nx + tmpl + (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 16));
 }
 
+// vectors per sub-batch: the per-launch scratch (row slices of `slice_doubles` doubles, templates, cell lists, lookup
+// series, partial tiles) stays under the context's budget (ppm_config.scratch_mb)
+static int compute_sb(const ppm_ctx* c, size_t slice_doubles)
+{
+    const ppm_config& g = c->cfg;
+    const double budget = (g.scratch_mb > 0 ? (double)g.scratch_mb : 1536.0) * 1048576.0;
+    const double per_row = (double)g.n_phase * g.n_energy * 8.0;
+    const double per_vec = (double)c->nchunk * per_row +
+                           (double)c->RT * ((double)slice_doubles * 8.0 + 4.0 * (c->n_fp + 1) * 8.0 + g.n_phi * 4.0 +
+                                            2.0 * kNCheb * 8.0 + (double)sizeof(RowD));
+    int sb = (int)std::max(1.0, std::min((double)g.max_batch, std::floor(budget / per_vec)));
+    return std::min(sb, 65535 / std::max(1, (g.n_energy + 31) / 32));      // grid.z limit with the smallest energy tile
+}
+
+static void free_scratch(ppm_ctx* c)
+{
+    void** ptrs[] = {(void**)&c->d_stars, (void**)&c->d_spots, (void**)&c->d_rows, (void**)&c->d_cells, (void**)&c->d_lookup,
+                     (void**)&c->d_tmpl, (void**)&c->d_partial, (void**)&c->d_pairs, (void**)&c->d_slices,
+                     (void**)&c->d_flux_stage, (void**)&c->d_counts_stage};
+    for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
+}
+
 static int alloc_scratch(ppm_ctx* c)
 {
     const ppm_config& g = c->cfg;
@@ -209,7 +231,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->n_theta >= 1 && cfg->n_phi >= 1 && cfg->n_phase >= 1 && cfg->n_energy >= 1, "grid sizes must be >= 1");
     ARG(cfg->n_fp >= 0, "n_fp must be >= 0");
     ARG(cfg->n_phi <= 12000, "n_phi must be <= 12000");
-    ARG(cfg->emission >= 0 && cfg->emission <= 3, "emission must be 0, 1, 2 or 3");
+    ARG(cfg->emission >= 0 && cfg->emission <= 4, "emission must be 0 .. 4");
     ARG(cfg->precision == 0 || cfg->precision == 1, "precision must be 0 (fp64) or 1 (fp32 interpolation + exponential)");
     ARG(cfg->precision == 0 || cfg->emission != PPM_EMISSION_BLACKBODY, "precision = 1 applies to table emission only");
     ARG(cfg->max_batch >= 1, "max_batch must be >= 1");
@@ -218,6 +240,9 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->mesh == 0 || cfg->mesh == 1, "mesh must be 0 (theta x phi box per spot) or 1 (HEALPix rings)");
     ARG(cfg->mesh == 0 || (cfg->n_phi % 4 == 0 && cfg->n_theta == cfg->n_phi - 1),
         "HEALPix mesh: n_phi = 4 N_side and n_theta = 4 N_side - 1");
+    ARG(cfg->scratch_mb >= 0, "scratch_mb must be >= 0");
+    ARG(cfg->phase_interp == 0 || cfg->phase_interp == 1, "phase_interp must be 0 / 1 (linear)");
+    ARG(cfg->interp_domain == 0, "interp_domain must be 0 (log10 I/T^3)");
     for (int e = 0; e < cfg->n_energy; ++e) {
         ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
         if (e) ARG(energies[e] > energies[e - 1], "energies must be strictly increasing");
@@ -229,6 +254,8 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ppm_ctx* c = new (std::nothrow) ppm_ctx;
     if (!c) { set_err("out of host memory"); return PPM_ERR_NOMEM; }
     c->cfg = *cfg;
+    // strategy b = strategy a + clipping of negative intensities; I = T^3 10^v > 0 when the logarithm is interpolated
+    if (cfg->emission == PPM_EMISSION_TABLE_CUBIC_CLIP && cfg->interp_domain == 0) c->cfg.emission = PPM_EMISSION_TABLE_CUBIC;
     c->stream = (cudaStream_t)stream;
     c->P = 8 + 8 * cfg->n_spots;
     c->RT = cfg->n_spots * cfg->n_theta;
@@ -248,11 +275,9 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     while ((double)((c->RT + c->rows_per_chunk - 1) / c->rows_per_chunk) * per_row > 96.0e6 && c->rows_per_chunk < c->RT)
         c->rows_per_chunk *= 2;
     c->nchunk = (c->RT + c->rows_per_chunk - 1) / c->rows_per_chunk;
-    // sub-batch: keep the per-launch scratch under ~1.5 GB
-    const double per_vec = (double)c->nchunk * per_row + (double)c->RT * (67.0 * 166.0 * 8.0 + 4.0 * (c->n_fp + 1) * 8.0 +
-                           cfg->n_phi * 4.0 + 2048.0);
-    c->SB = (int)std::max(1.0, std::min((double)cfg->max_batch, std::floor(1.5e9 / per_vec)));
-    c->SB = std::min(c->SB, 65535 / std::max(1, (cfg->n_energy + 31) / 32));     // grid.z limit with the smallest energy tile
+    // sub-batch: keep the per-launch scratch inside the budget; table emission re-sizes it in ppm_load_atmosphere
+    // once the slice size is known (blackbody emission has no slices)
+    c->SB = compute_sb(c, 0);
     int rc = alloc_scratch(c);
     if (rc) { ppm_destroy(c); return rc; }
     // energy-derived constants: filled here for blackbody; refreshed by ppm_load_atmosphere (needs h)
@@ -260,17 +285,23 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
         ppm_destroy(c);
         return rc;
     }
-    CK(cudaMemcpyAsync(c->d_en, energies, sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream));
     double glx[kNGL], glw[kNGL];
     gauss_legendre(kNGL, glx, glw);
-    CK(cudaMemcpyToSymbolAsync(c_glx, glx, sizeof(glx), 0, cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyToSymbolAsync(c_glw, glw, sizeof(glw), 0, cudaMemcpyHostToDevice, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
+    cudaError_t e = cudaMemcpyAsync(c->d_en, energies, sizeof(double) * cfg->n_energy, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbolAsync(c_glx, glx, sizeof(glx), 0, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbolAsync(c_glw, glw, sizeof(glw), 0, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) {
+        set_err("ppm_create: %s", cudaGetErrorString(e));
+        ppm_destroy(c);
+        return PPM_ERR_CUDA;
+    }
     *out = c;
     return PPM_OK;
 }
 
 extern "C" int ppm_n_fp(const ppm_ctx* c) { return c ? c->n_fp : 0; }
+extern "C" int ppm_sub_batch(const ppm_ctx* c) { return c ? c->SB : 0; }
 extern "C" int64_t ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }
 
 extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const double* logg, int ng,
@@ -291,6 +322,15 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     for (double** p : {&c->d_axT, &c->d_axg, &c->d_axmu, &c->d_values, &c->d_slices}) { if (*p) cudaFree(*p); *p = nullptr; }
     c->have_atm = false;
     int rc;
+    {   // the sub-batch follows the actual slice size (nmu x nx doubles per row)
+        const int sb = compute_sb(c, (size_t)nmu * nx);
+        if (sb != c->SB) {
+            CK(cudaStreamSynchronize(c->stream));
+            free_scratch(c);
+            c->SB = sb;
+            if ((rc = alloc_scratch(c))) return rc;
+        }
+    }
     const size_t nval = (size_t)nT * ng * nmu * nx;
     if ((rc = dev_alloc(&c->d_axT, (size_t)nT)) || (rc = dev_alloc(&c->d_axg, (size_t)ng)) ||
         (rc = dev_alloc(&c->d_axmu, (size_t)nmu)) || (rc = dev_alloc(&c->d_values, nval)) ||

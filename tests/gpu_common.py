@@ -18,10 +18,10 @@ def oracle_atm():
     return o.Atmosphere(*atmosphere())
 
 
-def make_ctx(conf, max_batch=None, precision=0):
+def make_ctx(conf, max_batch=None, precision=0, scratch_mb=0):
     import paper_2510_07764_b200 as ppm
     B = conf["params"].shape[0]
-    ctx = ppm.PPM(conf["cfg"], conf["energies"], max_batch=max_batch or B, precision=precision)
+    ctx = ppm.PPM(conf["cfg"], conf["energies"], max_batch=max_batch or B, precision=precision, scratch_mb=scratch_mb)
     if conf["cfg"]["emission"] != 0:
         ctx.load_atmosphere(*atmosphere())
     return ctx
@@ -50,3 +50,21 @@ def max_rel_err(g, ref):
     if not nz.any():
         return 0.0
     return float(np.max(np.abs(g[nz] - ref[nz]) / np.abs(ref[nz])))
+
+
+def chi2_eq56(model, ref):
+    """Eq 56-57 between two non-negative arrays: both scaled to a total of 1e6 'counts' of the
+    reference, chi^2 = K sum (m - d)^2 / m with m = reference (oracle), d = the other (GPU)."""
+    return o.chi2(np.asarray(ref, dtype=np.float64), np.asarray(model, dtype=np.float64))
+
+
+def report(name, **values):
+    """Append one line to gpurun_out/parity_report.jsonl (when that folder exists): the numbers DESIGN.md quotes."""
+    import json
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    d = os.path.join(root, "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, "parity_report.jsonl"), "a") as f:
+            f.write(json.dumps(dict(test=name, **{k: (float(v) if isinstance(v, (float, np.floating)) else v)
+                                                   for k, v in values.items()})) + "\n")
