@@ -9,7 +9,10 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
-LIB = os.path.join(_HERE, "libppm_b200.so")
+# PPM_BOUNDS=1 in the environment selects the debug build (-DPPM_BOUNDS: every shared-memory access of the table cell
+# kernel is checked against the block's allocation and traps outside it); it lives beside the product library.
+BOUNDS = os.environ.get("PPM_BOUNDS", "") not in ("", "0")
+LIB = os.path.join(_HERE, "libppm_b200_bounds.so" if BOUNDS else "libppm_b200.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -30,7 +33,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     srcs = sources()
     if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(s) for s in srcs):
         return LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (["-DPPM_BOUNDS"] if BOUNDS else []) + \
           ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB + ".tmp", os.path.join(CSRC, "ppm.cu")]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

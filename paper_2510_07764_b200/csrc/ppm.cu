@@ -114,6 +114,7 @@ struct ppm_ctx {
     bool have_atm = false;
     int nT = 0, ng = 0, nmu = 0, nx = 0;
     double x0 = 0, hx = 1;
+    double y_lo = 0, y_hi = 0;                    // bounds of log2(10) * (interpolated table value), see CellArgs
     double *d_axT = nullptr, *d_axg = nullptr, *d_axmu = nullptr, *d_values = nullptr;
     // response
     bool have_rsp = false;
@@ -179,10 +180,10 @@ extern "C" int ppm_destroy(ppm_ctx* c)
 // dynamic shared memory of the table cell kernels for `npl` nodes per lane (ppm_cells.cuh / ppm_cells32.cuh layouts)
 static size_t cells_tab_smem(const ppm_ctx* c, int nmu, int nx, int npl)
 {
-    const size_t tmpl = 4 * (size_t)(c->n_fp + 1) + nmu;
+    const size_t tmpl = 4 * (size_t)(c->n_fp + 1) + nmu + 16;            // + UG (first energy of each lane group)
     if (c->cfg.precision == 1)
         return sizeof(double) * (tmpl + (size_t)c->nw * (2 * 32 * npl + 64 + 64 + 16)) + sizeof(float) * ((size_t)nmu * nx + 32 * npl + 32);   // tail pad: out-of-window node reads stay inside
-    return sizeof(double) * ((size_t)nmu * nx + tmpl + (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 16));
+    return sizeof(double) * ((size_t)nmu * nx + tmpl + (size_t)c->nw * (4 * 32 * npl + 3 * 64 + 32));
 }
 
 // vectors per sub-batch: the per-launch scratch (row slices of `slice_doubles` doubles, templates, cell lists, lookup
@@ -241,7 +242,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
     ARG(cfg->mesh == 0 || (cfg->n_phi % 4 == 0 && cfg->n_theta == cfg->n_phi - 1),
         "HEALPix mesh: n_phi = 4 N_side and n_theta = 4 N_side - 1");
     ARG(cfg->scratch_mb >= 0, "scratch_mb must be >= 0");
-    ARG(cfg->phase_interp == 0 || cfg->phase_interp == 1, "phase_interp must be 0 / 1 (linear)");
+    ARG(cfg->phase_interp == 0 || cfg->phase_interp == 1 || cfg->phase_interp == 3, "phase_interp must be 0 / 1 (linear) or 3");
     ARG(cfg->interp_domain == 0, "interp_domain must be 0 (log10 I/T^3)");
     for (int e = 0; e < cfg->n_energy; ++e) {
         ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
@@ -341,6 +342,25 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
     CK(cudaMemcpyAsync(c->d_values, values, sizeof(double) * nval,
                        values_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     c->nT = nT; c->ng = ng; c->nmu = nmu; c->nx = nx; c->x0 = logx[0]; c->hx = h;
+    {   // range of the table -> bound of every interpolated value.  Lagrange weights can leave [0, 1]: the sum of their
+        // magnitudes is <= 1.25 per uniform cubic axis and stays below 2 on the non-uniform mu axis, so an interpolated value
+        // lies within (1.25^3 * 2 - 1) / 2 < 1.5 table ranges of [vmin, vmax]; 2 ranges are taken.
+        std::vector<double> hv;
+        const double* v = values;
+        if (values_on_device) {
+            hv.resize(nval);
+            CK(cudaMemcpy(hv.data(), values, sizeof(double) * nval, cudaMemcpyDeviceToHost));
+            v = hv.data();
+        }
+        double vmin = v[0], vmax = v[0];
+        for (size_t i = 0; i < nval; ++i) {
+            ARG(std::isfinite(v[i]), "table values must be finite");
+            vmin = std::min(vmin, v[i]); vmax = std::max(vmax, v[i]);
+        }
+        const double range = vmax - vmin;
+        c->y_lo = kLog2_10 * (vmin - 2.0 * range);
+        c->y_hi = kLog2_10 * (vmax + 2.0 * range);
+    }
     std::vector<double> ue(c->cfg.n_energy);
     for (int e = 0; e < c->cfg.n_energy; ++e) ue[e] = std::log10(c->h_en[e]) / h;
     std::vector<long long> uef(c->cfg.n_energy);
@@ -546,6 +566,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh; A.beaming = g.beaming;
+    A.phase_order = g.phase_interp == 3 ? 3 : 1; A.y_lo = c->y_lo; A.y_hi = c->y_hi;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     int rc;

@@ -29,6 +29,9 @@ struct CellArgs {
     int nmu, nx, mu_rule, x_linedge;
     int nchunk, rows_per_chunk, nw, n_etile, mesh;
     int beaming;             // blackbody only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma')
+    int phase_order;         // Interp of Eq 46: 1 linear (reading R11), 3 four-point Lagrange (reading R11b)
+    double y_lo, y_hi;       // bounds of log2(10) * (any interpolated table value): a pair whose log2(F_p T^3) + y_lo
+                             // < -900 or + y_hi > 900 takes the range-checked energy loop (exponent add must not wrap)
 };
 
 // ---- K4: collapse the 4-D table to the row's (mu x logx) slice: T is per spot, g per row -------
@@ -65,18 +68,104 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
 // 2^f by a degree-8 polynomial (Chebyshev-node fit on [-1/2, 1/2]; max relative error 1.1e-12 -- three orders
 // below the 1e-9 per-bin parity bar; degree 10 reaches 4e-16 at +2 DFMA per triple, measured 6 % slower),
 // 2^n by an integer add into the exponent field.  The caller drops terms with n < -1000.
+// The coefficients sit in the constant bank: every DFMA of the Horner chain takes its addend straight from c[][]
+// (no register, no per-pair re-materialisation of 18 words).
+__constant__ double c_exp2[9] = {1.3255224878668817e-06, 1.5310079402249296e-05, 0.00015403455852453838,
+                                 0.0013333450568000645,  0.009618129159402558,   0.05550410941205933,
+                                 0.2402265069581299,     0.6931471805459335,     1.0};
+
 __device__ __forceinline__ double exp2_frac_scaled(double f, int n)      // 2^f * 2^n, |f| <= 1/2, no range check
 {
-    double p = 1.3255224878668817e-06;
-    p = fma(p, f, 1.5310079402249296e-05);
-    p = fma(p, f, 0.00015403455852453838);
-    p = fma(p, f, 0.0013333450568000645);
-    p = fma(p, f, 0.009618129159402558);
-    p = fma(p, f, 0.05550410941205933);
-    p = fma(p, f, 0.2402265069581299);
-    p = fma(p, f, 0.6931471805459335);
-    p = fma(p, f, 1.0);
+    double p = c_exp2[0];
+    p = fma(p, f, c_exp2[1]);
+    p = fma(p, f, c_exp2[2]);
+    p = fma(p, f, c_exp2[3]);
+    p = fma(p, f, c_exp2[4]);
+    p = fma(p, f, c_exp2[5]);
+    p = fma(p, f, c_exp2[6]);
+    p = fma(p, f, c_exp2[7]);
+    p = fma(p, f, c_exp2[8]);
     return __hiloint2double(__double2hiint(p) + n * 1048576, __double2loint(p));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step A of every cell kernel: one lane <-> one (cell, output phase) slot.
+// phase_of_cell: Eq 45.  template_interp: the bracket phi_o[i] <= phi_p < phi_o[i+1] and Interp of
+// Eq 46 -- ORDER 1: piecewise linear (reading R11); ORDER 3: 4-point Lagrange on the true
+// abscissae phi_o with periodic wrap, reverting to linear when one of the four F nodes is 0 (a hidden or filled
+// entry, Eq 41; reading R11b).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double phase_of_cell(double phi_out, double phi_m, double phi_off, double po0)
+{
+    const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
+    return (s0 - floor(s0)) + po0;
+}
+
+__device__ __forceinline__ void template_interp(const double* __restrict__ F, const double* __restrict__ Z,
+                                                const double* __restrict__ PO, const double* __restrict__ MU, int n_fp,
+                                                int order, double phi_p, double& Fp, double& zp, double& mup)
+{
+    int lo = 0, hi = n_fp;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (PO[mid] <= phi_p) lo = mid; else hi = mid;
+    }
+    if (order == 3) {
+        const int i0 = (lo == 0) ? n_fp - 1 : lo - 1, i3 = (lo + 2 > n_fp) ? 1 : lo + 2;
+        const double f0 = F[i0], f1 = F[lo], f2 = F[lo + 1], f3 = F[i3];
+        if (f0 != 0.0 && f1 != 0.0 && f2 != 0.0 && f3 != 0.0) {
+            const double x0 = PO[i0] + ((lo == 0) ? -1.0 : 0.0), x1 = PO[lo], x2 = PO[lo + 1];
+            const double x3 = PO[i3] + ((lo + 2 > n_fp) ? 1.0 : 0.0);
+            const double d0 = phi_p - x0, d1 = phi_p - x1, d2 = phi_p - x2, d3 = phi_p - x3;
+            const double w0 = (d1 * d2 * d3) / ((x0 - x1) * (x0 - x2) * (x0 - x3));
+            const double w1 = (d0 * d2 * d3) / ((x1 - x0) * (x1 - x2) * (x1 - x3));
+            const double w2 = (d0 * d1 * d3) / ((x2 - x0) * (x2 - x1) * (x2 - x3));
+            const double w3 = (d0 * d1 * d2) / ((x3 - x0) * (x3 - x1) * (x3 - x2));
+            Fp = fma(w3, f3, fma(w2, f2, fma(w1, f1, w0 * f0)));
+            zp = fma(w3, Z[i3], fma(w2, Z[lo + 1], fma(w1, Z[lo], w0 * Z[i0])));
+            mup = fma(w3, MU[i3], fma(w2, MU[lo + 1], fma(w1, MU[lo], w0 * MU[i0])));
+            return;
+        }
+    }
+    const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
+    Fp = F[lo] + (F[lo + 1] - F[lo]) * t;
+    zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
+    mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+}
+
+// azimuth of cell m of a row (box mesh, reading R1; HEALPix ring, Eq 24-27)
+__device__ __forceinline__ double cell_azimuth(int mesh, const RowD& row, const SpotD& sp, int m)
+{
+    return mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
+}
+
+// flags of a pair record (int2.y); bits 8.. hold the number of energy groups that still need per-triple work when only
+// PAIR_CLAMP_HI is set (see k_cells_tab)
+enum { PAIR_CLAMP_LO = 1, PAIR_CLAMP_HI = 2, PAIR_RANGE = 4 };
+
+// The table part of a pair record: logx coordinate of the pair in fixed point (units of 2^-52 intervals; the energy
+// part uef[e] is added per triple), log2(F_p T^3), the mu stencil (weights pre-scaled by log2(10)), the window of logx
+// intervals [jlo, jhi] the tile's energies touch (coordinates clamped to the table, reading R13b) and the flags.
+//   info = (first mu row of the stencil * row_stride) | jlo << 16 | jhi << 24
+__device__ __forceinline__ void pair_table_record(double Fp, double zp, double mup, double log10kT, double log2T3,
+                                                  const double* __restrict__ MUAX, int nmu, int mu_rule, int row_stride,
+                                                  double inv_h, double x0_over_h, long long uef_first,
+                                                  long long uef_last, long long s_top, double y_lo, double y_hi,
+                                                  long long& pq, double& pb, double ww[4], int& info, int& flags)
+{
+    const double up = (log10(zp) - log10kT) * inv_h - x0_over_h;                 // (x - x0)/h less the energy part
+    pq = __double2ll_rn(up * 4503599627370496.0);
+    pb = log2(Fp) + log2T3;
+    int mb;
+    axis_w4(MUAX, nmu, mup, mu_rule, mb, ww);
+#pragma unroll
+    for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= kLog2_10;
+    const long long sa = pq + uef_first, sb2 = pq + uef_last;
+    const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
+    const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
+    info = (mb * row_stride) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24);
+    flags = (sa < 0 ? PAIR_CLAMP_LO : 0) | (sb2 > s_top ? PAIR_CLAMP_HI : 0) |
+            ((!(pb + y_lo > -900.0) || !(pb + y_hi < 900.0)) ? PAIR_RANGE : 0);
 }
 
 
@@ -137,25 +226,14 @@ __global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
             const int idx = base + lane;
             double Fp = 0.0, pa = 0.0, pb = 0.0;      // pa = z_p / kT, pb = F_p z_p^3 2/(h^3 c^2)
             if (idx < nact) {
-                const int m = cl[idx];
-                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
-                const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
-                const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
-                int lo = 0, hi = A.n_fp;
-                while (hi - lo > 1) {
-                    const int mid = (lo + hi) >> 1;
-                    if (PO[mid] <= phi_p) lo = mid; else hi = mid;
-                }
-                const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
-                Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                           // Eq 46, linear (reading R11)
-                const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
+                const double phi_p = phase_of_cell(phi_out, cell_azimuth(A.mesh, row, sp, cl[idx]), phi_off, po0);   // Eq 45
+                double zp, mup;
+                template_interp(F, Z, PO, MU, A.n_fp, A.phase_order, phi_p, Fp, zp, mup);                            // Eq 46
+                if (!(Fp > 0.0)) Fp = 0.0;
                 if (Fp != 0.0) {
                     pa = zp / sp.kT;
                     pb = Fp * (2.0 / (kH_keV_s * kH_keV_s * kH_keV_s * kC_cm_s * kC_cm_s)) * zp * zp * zp;
-                    if (A.beaming) {                                            // cos(sigma') = mu_p (Eq 20)
-                        const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
-                        pb *= (A.beaming == 1) ? mup * mup : 1.0 - mup * mup;
-                    }
+                    if (A.beaming) pb *= (A.beaming == 1) ? mup * mup : 1.0 - mup * mup;      // cos(sigma') = mu_p (Eq 20)
                 }
             }
             unsigned todo = __ballot_sync(0xffffffffu, Fp != 0.0);
@@ -233,6 +311,75 @@ __device__ __forceinline__ void cubic_coeffs(double c0, double c1, double c2, do
     k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
 }
 
+// debug build (-DPPM_BOUNDS): every shared-memory access of the table cell kernel is checked against the block's
+// dynamic allocation and traps when it falls outside (compute-sanitizer is not available on the GPU pool)
+#ifdef PPM_BOUNDS
+__device__ __forceinline__ void smem_check(const void* p, size_t bytes, const void* base)
+{
+    unsigned dyn;
+    asm volatile("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+    const char* c = static_cast<const char*>(p);
+    const char* b = static_cast<const char*>(base);
+    if (c < b || c + bytes > b + dyn) __trap();
+}
+#define PPM_SMEM_CHECK(p, bytes) smem_check((p), (bytes), sm)
+#else
+#define PPM_SMEM_CHECK(p, bytes) ((void)0)
+#endif
+
+// one triple: logx coordinate s (fixed point) -> interval coefficients -> y -> 2^y (no range checks)
+template <int KW>
+__device__ __forceinline__ double triple_value(const double2* __restrict__ KAq, long long s)
+{
+    const int shi = (int)(s >> 32);
+    const double2* kp = KAq + (shi >> 20);                                      // interval index = s >> 52
+    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+    const double2 c01 = kp[0], c23 = kp[KW];
+    const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+    const double r = y + kMagic;
+    return exp2_frac_scaled(y - (r - kMagic), __double2loint(r));
+}
+
+// the same with the coordinate clamped to the table (reading R13b) and the exponent range checked on both sides:
+// below 2^-1000 the term is 0, above 2^1000 it is +inf (the exponent add of exp2_frac_scaled would wrap)
+template <int KW>
+__device__ __forceinline__ double triple_value_checked(const double2* __restrict__ KAq, long long s, long long s_top)
+{
+    s = s < 0 ? 0 : (s > s_top ? s_top : s);
+    const int shi = (int)(s >> 32);
+    const double2* kp = KAq + (shi >> 20);
+    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+    const double2 c01 = kp[0], c23 = kp[KW];
+    const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+    const double r = y + kMagic;
+    const int n = __double2loint(r);
+    const double v = exp2_frac_scaled(y - (r - kMagic), n);
+    return !(y > -1000.0) ? 0.0 : (y > 1000.0 ? INFINITY : v);
+}
+
+// Energies of a pair whose upper part lies beyond the top of the logx axis.  The lane's energies e0 + lane + 32 i rise
+// with i and with the lane, so the groups i >= G (G warp-uniform: the groups whose FIRST energy is still inside the table)
+// are clamped for every lane: their term is the pair's constant 2^y(s_top) and is not evaluated here (the caller defers it).
+// Groups i < G - 1 are entirely inside the table; group G - 1 may straddle the end and clamps its coordinate.
+// One fully unrolled instance per G keeps the G independent dependency chains interleaved.
+template <int KW, int EPL, int G>
+__device__ __forceinline__ void energies_clamped_hi(double (&acc)[EPL], const long long (&uef)[EPL],
+                                                    const double2* __restrict__ KAq, long long q, long long s_top)
+{
+#pragma unroll
+    for (int i = 0; i < G - 1; ++i) acc[i] += triple_value<KW>(KAq, q + uef[i]);
+    const long long s = q + uef[G - 1];
+    acc[G - 1] += triple_value<KW>(KAq, s > s_top ? s_top : s);
+}
+
+template <int KW, int EPL, int G>
+__device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], const long long (&uef)[EPL],
+                                                    const double2* __restrict__ KAq, long long q, long long s_top)
+{
+    if (g == G) energies_clamped_hi<KW, EPL, G>(acc, uef, KAq, q, s_top);
+    else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1>(g, acc, uef, KAq, q, s_top);
+}
+
 template <int EPL, int NPL>
 __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
@@ -247,19 +394,20 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
     const int nx = A.nx;
     const int plane = A.nmu * nx;
     // shared layout (doubles): per warp { KA [KW] (k0,k1), KB [KW] (k2,k3), R0 [32] (q,qb), R1 [32] (v0,v1), R2 [32] (v2,v3)
-    // as double2, RI [32] int } | S [nmu][nx] | T [4][n1] | MUAX [nmu].  Struct-of-arrays so that lanes touch consecutive
-    // 16-byte words (no bank conflicts); KA / KB are indexed by node offset inside the pair's window.
+    // as double2, RI [32] int2 (info, flags) } | S [nmu][nx] | T [4][n1] | MUAX [nmu].  Struct-of-arrays so that lanes
+    // touch consecutive 16-byte words (no bank conflicts); KA / KB are indexed by node offset inside the pair's window.
     constexpr int KW = 32 * NPL;
-    constexpr int WARP_DBL = 4 * KW + 3 * 64 + 16;
+    constexpr int WARP_DBL = 4 * KW + 3 * 64 + 32;
     double* wbase = sm + (size_t)w * WARP_DBL;
     double2* KA = reinterpret_cast<double2*>(wbase);
     double2* R0 = KA + 2 * KW;
     double2* R1 = R0 + 32;
     double2* R2 = R1 + 32;
-    int* RI = reinterpret_cast<int*>(R2 + 32);
+    int2* RI = reinterpret_cast<int2*>(R2 + 32);
     double* S = sm + (size_t)A.nw * WARP_DBL;
     double* T = S + plane;
     double* MUAX = T + 4 * n1;
+    long long* UG = reinterpret_cast<long long*>(MUAX + A.nmu);                 // [EPL]: coordinate part of each group's first energy
 
     long long uef[EPL];
     double acc[EPL];
@@ -269,10 +417,13 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
         uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
         acc[i] = 0.0;
     }
+    double hdef = 0.0;                           // lane g: sum of the constants 2^y(s_top) of the pairs whose groups >= g are clamped
     const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
     const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
     const long long s_top = ((long long)(nx - 1) << 52) - 1;                     // largest in-table coordinate
     for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
+    if (threadIdx.x < EPL)                       // a group without any energy (ragged tail) counts as beyond the table
+        UG[threadIdx.x] = (e0 + 32 * threadIdx.x < A.nE) ? A.uef[e0 + 32 * threadIdx.x] : (1ll << 62);
 
     const StarD& st = A.stars[b];
     const double phi_off = st.phi_off;
@@ -314,35 +465,21 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
             double Fp = 0.0, pb = 0.0;                // pb = log2(F_p T^3)
             long long pq = 0;                         // u_pair in units of 2^-52 intervals
             double ww[4] = {0.0, 0.0, 0.0, 0.0};
-            int info = 0;                             // slice offset of the mu stencil's first row | jlo << 16 | jhi << 24
+            int info = 0, flags = 0;
             if (idx < nact) {
-                const int m = cl[idx];
-                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
-                const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
-                const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
-                int lo = 0, hi = A.n_fp;
-                while (hi - lo > 1) {
-                    const int mid = (lo + hi) >> 1;
-                    if (PO[mid] <= phi_p) lo = mid; else hi = mid;
-                }
-                const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
-                Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                           // Eq 46, linear (reading R11)
-                const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
-                const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+                const double phi_p = phase_of_cell(phi_out, cell_azimuth(A.mesh, row, sp, cl[idx]), phi_off, po0);   // Eq 45
+                double zp, mup;
+                template_interp(F, Z, PO, MU, A.n_fp, A.phase_order, phi_p, Fp, zp, mup);                            // Eq 46
+                if (!(Fp > 0.0)) Fp = 0.0;
                 if (Fp != 0.0) {
-                    const double up = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h;   // (x - x0)/h less the energy part
-                    pq = __double2ll_rn(up * kTwo52);
-                    pb = log2(Fp) + sp.log2T3;
-                    int mb;
-                    axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
+                    pair_table_record(Fp, zp, mup, sp.log10kT, sp.log2T3, MUAX, A.nmu, A.mu_rule, nx, A.inv_h, A.x0_over_h,
+                                      uef_first, uef_last, s_top, A.y_lo, A.y_hi, pq, pb, ww, info, flags);
+                    if (flags == PAIR_CLAMP_HI) {                               // groups whose first energy is inside the table
+                        int g = 0;
 #pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= kLog2_10;
-                    // window of logx intervals touched by this pair's energies (coordinates clamped to the table, reading R13b)
-                    const long long sa = pq + uef_first, sb2 = pq + uef_last;
-                    const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
-                    const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
-                    const int clamped = (sa < 0) || (sb2 > s_top);
-                    info = (mb * nx) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
+                        for (int i = 0; i < EPL; ++i) g += (pq + UG[i] <= s_top) ? 1 : 0;
+                        flags |= g << 8;
+                    }
                 }
             }
             const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);
@@ -354,22 +491,24 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 R0[slot] = make_double2(__longlong_as_double(pq), pb);
                 R1[slot] = make_double2(ww[0], ww[1]);
                 R2[slot] = make_double2(ww[2], ww[3]);
-                RI[slot] = info;
+                RI[slot] = make_int2(info, flags);
             }
             __syncwarp();
             // ---- step B: walk the valid pairs ----
             for (int pj = 0; pj < cnt; ++pj) {
                 const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj];
-                const int inf = RI[pj];
+                const int2 ri2 = RI[pj];
+                const int inf = ri2.x, flg = ri2.y;
                 const long long q = __double_as_longlong(r0.x);
                 const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                 const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
-                const double* srow = S + (inf & 0x7FFF);
+                const double* srow = S + (inf & 0xFFFF);
                 // ---- fused pass: node values -> interval coefficients.  Lane l holds nodes n0 .. n0+NPL-1, n0 = jlo-1 + NPL l;
                 // interval c (nodes c, c+1) has window offset c - (jlo-1).  Out-of-table nodes read neighbouring shared memory:
                 // they only feed window slots that no energy reads.
                 const int n0 = jlo - 1 + NPL * lane;
                 const double* sp0 = srow + n0;
+                PPM_SMEM_CHECK(sp0, sizeof(double) * (3 * nx + NPL));
                 double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
 #pragma unroll
                 for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node_value(sp0 + jn, nx, v0, v1, v2, v3, qb);
@@ -405,12 +544,6 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         }
                     }
                 }
-                // terms below 2^-900 (possible only with extreme table values) take the guarded loop: the exponent add of
-                // exp2_frac_scaled must not wrap.  k0 is the exponent at the interval midpoint; +-100 covers the interval.
-                bool tiny = false;
-#pragma unroll
-                for (int jn = 0; jn < NPL; ++jn) tiny |= (n0 + jn >= jlo) && (n0 + jn <= jhi) && !(ka[jn].x > -800.0);
-                const bool guarded = __any_sync(0xffffffffu, tiny) || (inf & 0x8000);
                 __syncwarp();                                                   // the previous pair's readers are done
 #pragma unroll
                 for (int jn = 0; jn < NPL; ++jn) {
@@ -420,40 +553,40 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 __syncwarp();
                 const double2* KAq = KA + (1 - jlo);
                 // ---- energies ----
-                if (!guarded) {
+                if (flg == 0) {
+                    // every coordinate of the tile lies inside the table and every exponent is in range
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
-                        const long long s = q + uef[i];
-                        const int shi = (int)(s >> 32);
-                        const double2* kp = KAq + (shi >> 20);                  // interval index = s >> 52
-                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
-                        const double2 c01 = kp[0], c23 = kp[KW];
-                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
-                        const double r = y + kMagic;
-                        const int n = __double2loint(r);
-                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        acc[i] += val;
+                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52), sizeof(double2));
+                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52) + KW, sizeof(double2));
+                        acc[i] += triple_value<KW>(KAq, q + uef[i]);
                     }
+                } else if ((flg & 7) == PAIR_CLAMP_HI) {
+                    // the upper energies lie beyond the top of the logx axis: the clamped coordinate (reading R13b) makes
+                    // their term the pair's constant 2^y(s_top).  Groups g .. EPL-1 (g = flg >> 8) are clamped for every lane:
+                    // the constant goes to lane g's deferred sum and is spread over acc[g ..] once, in the epilogue.
+                    const int g = flg >> 8;
+                    const double vtop = triple_value<KW>(KAq, s_top);
+                    if (lane == g) hdef += vtop;
+                    dispatch_clamped_hi<KW, EPL, EPL>(g, acc, uef, KAq, q, s_top);
                 } else {
+                    // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
+                    // range-checked form
 #pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        long long s = q + uef[i];
-                        s = s < 0 ? 0 : (s > s_top ? s_top : s);                 // clamp to the table (reading R13b)
-                        const int shi = (int)(s >> 32);
-                        const double2* kp = KAq + (shi >> 20);
-                        const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
-                        const double2 c01 = kp[0], c23 = kp[KW];
-                        const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
-                        const double r = y + kMagic;
-                        const int n = __double2loint(r);
-                        const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                        if (n >= -1000) acc[i] += val;       // below: the exponent add wrapped, the term is 0
-                    }
+                    for (int i = 0; i < EPL; ++i) acc[i] += triple_value_checked<KW>(KAq, q + uef[i], s_top);
                 }
             }
         }
     }
     if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
+    // deferred constants of the clamped groups: acc[i] += sum over g <= i of lane g's hdef (inclusive scan over lanes)
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const double up = __shfl_up_sync(0xffffffffu, hdef, d);
+        if (lane >= d) hdef += up;
+    }
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, i);
     if (kvalid) {
         double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
 #pragma unroll

@@ -146,30 +146,17 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab32(CellArgs A)
             double ww[4] = {0.0, 0.0, 0.0, 0.0};
             int info = 0;
             if (idx < nact) {
-                const int m = cl[idx];
-                const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
-                const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
-                const double phi_p = (s0 - floor(s0)) + po0;                    // Eq 45
-                int lo = 0, hi = A.n_fp;
-                while (hi - lo > 1) {
-                    const int mid = (lo + hi) >> 1;
-                    if (PO[mid] <= phi_p) lo = mid; else hi = mid;
-                }
-                const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
-                Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                           // Eq 46, linear (reading R11)
-                const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
-                const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
+                const double phi_p = phase_of_cell(phi_out, cell_azimuth(A.mesh, row, sp, cl[idx]), phi_off, po0);   // Eq 45
+                double zp, mup;
+                template_interp(F, Z, PO, MU, A.n_fp, A.phase_order, phi_p, Fp, zp, mup);                            // Eq 46
+                if (!(Fp > 0.0)) Fp = 0.0;
                 if (Fp != 0.0) {
-                    const double up = (log10(zp) - sp.log10kT) * A.inv_h - A.x0_over_h;
-                    pq = __double2ll_rn(up * kTwo52);
-                    pb = log2(Fp) + sp.log2T3 - (double)n_row;                  // relative to the row exponent
-                    int mb;
-                    axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
-                    const long long sa = pq + uef_first, sb2 = pq + uef_last;
-                    const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
-                    const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
-                    const int clamped = (sa < 0) || (sb2 > s_top);
-                    info = (mb * nx) | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
+                    int flags;
+                    pair_table_record(Fp, zp, mup, sp.log10kT, sp.log2T3 - (double)n_row, MUAX, A.nmu, A.mu_rule, nx, A.inv_h,
+                                      A.x0_over_h, uef_first, uef_last, s_top, 0.0, 0.0, pq, pb, ww, info, flags);
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= 1.0 / kLog2_10;         // the FP32 slice is already scaled by log2(10)
+                    if (flags & (PAIR_CLAMP_LO | PAIR_CLAMP_HI)) info |= 0x8000;
                 }
             }
             const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);

@@ -178,35 +178,16 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                     const double lT = tcell[m];
                     double tt;
                     axis_linear(TAX, A.nT, lT, tt);
-                    {
-                        const double phi_m = A.mesh ? row.phi0 + (double)m * row.dphi
-                                                    : sp.phi_c + (-sp.W + ((double)m + 0.5) * sp.dphi);
-                        const double s0 = phi_out + phi_m / (2.0 * kPi) + phi_off + 1.0 - po0;
-                        const double phi_p = (s0 - floor(s0)) + po0;                // Eq 45
-                        int lo = 0, hi = A.n_fp;
-                        while (hi - lo > 1) {
-                            const int mid = (lo + hi) >> 1;
-                            if (PO[mid] <= phi_p) lo = mid; else hi = mid;
-                        }
-                        const double t = (phi_p - PO[lo]) / (PO[lo + 1] - PO[lo]);
-                        Fp = F[lo] + (F[lo + 1] - F[lo]) * t;                       // Eq 46, linear (reading R11)
-                        const double zp = Z[lo] + (Z[lo + 1] - Z[lo]) * t;
-                        const double mup = MU[lo] + (MU[lo + 1] - MU[lo]) * t;
-                        if (Fp != 0.0) {
-                            const double up = (log10(zp) - (log10kB + lT)) * A.inv_h - A.x0_over_h;
-                            pq = __double2ll_rn(up * kTwo52);
-                            pb = log2(Fp) + 3.0 * lT * kLog2_10;                    // log2(F_p T^3), T of this cell
-                            tw = tt;
-                            int mb;
-                            axis_w4(MUAX, A.nmu, mup, A.mu_rule, mb, ww);
-#pragma unroll
-                            for (int q4 = 0; q4 < 4; ++q4) ww[q4] *= kLog2_10;
-                            const long long sa = pq + uef_first, sb2 = pq + uef_last;
-                            const long long sac = sa < 0 ? 0 : (sa > s_top ? s_top : sa);
-                            const long long sbc = sb2 < 0 ? 0 : (sb2 > s_top ? s_top : sb2);
-                            const int clamped = (sa < 0) || (sb2 > s_top);
-                            info = mb | ((int)(sac >> 52) << 16) | ((int)(sbc >> 52) << 24) | (clamped << 15);
-                        }
+                    const double phi_p = phase_of_cell(phi_out, cell_azimuth(A.mesh, row, sp, m), phi_off, po0);   // Eq 45
+                    double zp, mup;
+                    template_interp(F, Z, PO, MU, A.n_fp, A.phase_order, phi_p, Fp, zp, mup);                  // Eq 46
+                    if (!(Fp > 0.0)) Fp = 0.0;
+                    if (Fp != 0.0) {
+                        int flags;                                                  // T, kT, T^3 of this cell
+                        pair_table_record(Fp, zp, mup, log10kB + lT, 3.0 * lT * kLog2_10, MUAX, A.nmu, A.mu_rule, 1, A.inv_h,
+                                          A.x0_over_h, uef_first, uef_last, s_top, 0.0, 0.0, pq, pb, ww, info, flags);
+                        if (flags & (PAIR_CLAMP_LO | PAIR_CLAMP_HI)) info |= 0x8000;
+                        tw = tt;
                     }
                 }
                 const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);

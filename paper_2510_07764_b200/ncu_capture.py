@@ -21,15 +21,17 @@ UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
         "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "s": 1.0, "usecond": 1e-6, "nsecond": 1e-9, "msecond": 1e-3, "second": 1.0}
 
 WANT = {
-    "dfma": "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum",
-    "dadd": "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum",
-    "dmul": "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum",
-    "ffma": "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum",
-    "fadd": "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum",
-    "fmul": "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum",
+    # thread-level instruction counts: `--set full` reports them per elapsed cycle; parse() multiplies by smsp_cycles
+    "dfma_per_cycle": "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum.per_cycle_elapsed",
+    "dadd_per_cycle": "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum.per_cycle_elapsed",
+    "dmul_per_cycle": "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum.per_cycle_elapsed",
+    "ffma_per_cycle": "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum.per_cycle_elapsed",
+    "fadd_per_cycle": "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum.per_cycle_elapsed",
+    "fmul_per_cycle": "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum.per_cycle_elapsed",
+    "smsp_cycles": "smsp__cycles_elapsed.avg",
+    "l2_sectors": "lts__t_sectors.sum",
     "dram_read_bytes": "dram__bytes_read.sum",
     "dram_write_bytes": "dram__bytes_write.sum",
-    "l2_bytes": "lts__t_bytes.sum",
     "time_s": "gpu__time_duration.sum",
     "cycles": "sm__cycles_elapsed.max",
     "inst_executed": "smsp__inst_executed.sum",
@@ -72,6 +74,11 @@ def parse(path, kernel):
                     except ValueError:
                         continue
                     out[k] = v * UNIT.get(units[j], 1.0)
+            for op in ("dfma", "dadd", "dmul", "ffma", "fadd", "fmul"):
+                if op + "_per_cycle" in out and "smsp_cycles" in out:
+                    out[op] = out.pop(op + "_per_cycle") * out["smsp_cycles"]
+            if "l2_sectors" in out:
+                out["l2_bytes"] = 32.0 * out["l2_sectors"]
             return out
     raise SystemExit("no launch of %s in %s" % (kernel, path))
 
