@@ -69,6 +69,12 @@ def workload(name, batch, rank, world=1):
         if name == "T":
             desc = "north-star target T = vector 0 of C5 evaluated alone; " + desc
         return conf, desc
+    if name in ("I1", "I2"):
+        conf = gen.config_interp_test(int(name[1]), n_cells=256, n_phase=128, n_energy=128)
+        conf["params"] = np.ascontiguousarray(np.repeat(conf["params"], batch, axis=0))
+        conf["steep_table"] = True
+        return conf, ("interpolation test %s of Table 3 (PAPER.md:520-533): point-like spot, 256x256 cells, 128 phases x 128 "
+                      "energies (Eq 50 grid), steep-limb synthetic table, batch of %d identical vectors per GPU" % (name[1], batch))
     conf = {"C1": gen.config_c1, "C2": gen.config_c2, "C3": gen.config_c3, "C4": gen.config_c4}[name]()
     conf["params"] = np.ascontiguousarray(np.repeat(conf["params"], batch, axis=0))
     idx = {"C1": 0, "C2": 1, "C3": 2, "C4": 3}[name]
@@ -147,7 +153,8 @@ def oracle_sample(conf, n_extra=4, threads=None):
     linear extrapolation to n_phase phases.  -> dict(value evals/s, seconds, cores, sample)."""
     import oracle as o
     cfg, E = conf["cfg"], conf["energies"]
-    atm = o.Atmosphere(*gen.synthetic_atmosphere()) if cfg["emission"] else None
+    atm = o.Atmosphere(*(gen.steep_limb_atmosphere() if conf.get("steep_table") else gen.synthetic_atmosphere())) \
+        if cfg["emission"] else None
     nph = cfg["n_phase"]
     n_extra = max(1, min(n_extra, nph - 1))
     sel1 = [nph // 3]
@@ -173,7 +180,8 @@ def oracle_full(conf, threads=None):
     """One whole evaluation of vector 0 by the CPU oracle (+ fold + ln L where the workload has a response)."""
     import oracle as o
     cfg, E = conf["cfg"], conf["energies"]
-    atm = o.Atmosphere(*gen.synthetic_atmosphere()) if cfg["emission"] else None
+    atm = o.Atmosphere(*(gen.steep_limb_atmosphere() if conf.get("steep_table") else gen.synthetic_atmosphere())) \
+        if cfg["emission"] else None
     rsp = gen.synthetic_response(E) if len(E) == 300 else None
     all_threads = o.num_threads()
     if threads:
@@ -257,7 +265,12 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ppm", choices=["ppm", "reference"])
-    ap.add_argument("--workload", default="C5", choices=["C5", "T", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C5", choices=["C5", "T", "C1", "C2", "C3", "C4", "I1", "I2"])
+    ap.add_argument("--emission", type=int, default=None, choices=[1, 2, 3, 4],
+                    help="override the workload's interpolation strategy: 1 a, 4 b, 3 c, 2 d (PAPER.md:551)")
+    ap.add_argument("--interp-domain", type=int, default=0, choices=[0, 1],
+                    help="1: the table interpolation acts on I/T^3 instead of its logarithm (reading R13g)")
+    ap.add_argument("--phase-interp", type=int, default=0, choices=[0, 1, 3], help="order of Interp in Eq 46 (reading R11b)")
     ap.add_argument("--batch", type=int, default=8,
                     help="parameter vectors per GPU and step (C5: BASELINE.json states 1024; the default 8 gives the "
                          "per-evaluation figure in seconds instead of minutes)")
@@ -291,11 +304,15 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     conf, desc = workload(args.workload, args.batch, rank, world)
+    if args.emission is not None and conf["cfg"]["emission"]:
+        conf["cfg"] = dict(conf["cfg"], emission=args.emission)
+    conf["cfg"] = dict(conf["cfg"], interp_domain=args.interp_domain if conf["cfg"]["emission"] else 0,
+                       phase_interp=args.phase_interp)
     cfg, E = conf["cfg"], conf["energies"]
     B = conf["params"].shape[0]
     ctx = ppm.PPM(cfg, E, max_batch=B, device=local, precision=args.precision)
     if cfg["emission"]:
-        ctx.load_atmosphere(*gen.synthetic_atmosphere())
+        ctx.load_atmosphere(*(gen.steep_limb_atmosphere() if conf.get("steep_table") else gen.synthetic_atmosphere()))
     rsp = gen.synthetic_response(E)
     ctx.set_response(rsp["n_channel"], rsp["first_chan"], rsp["rsp_band"], rsp["tau_ref"])
     data_h, bkg_h = gen.synthetic_counts(cfg["n_phase"], rsp["n_channel"])
@@ -392,9 +409,12 @@ def main():
             peak_dfma = None
         kern_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
         table = bool(cfg["emission"])
-        kname = (("k_cells_map" if args.tmap is not None else "k_cells_tab32" if args.precision else "k_cells_tab")
+        kname = (("k_cells_map" if args.tmap is not None else "k_cells_lin" if args.interp_domain else
+                  "k_cells_tab32" if args.precision else "k_cells_tab")
                  if table else "k_cells_bb")
         key = "%s:%d:p%d%s" % (args.workload, B, args.precision, "" if args.tmap is None else ":tmap%g" % args.tmap)
+        if args.emission is not None or args.interp_domain or args.phase_interp == 3:
+            key += ":e%s:d%d:ph%d" % (args.emission, args.interp_domain, args.phase_interp)
         cap = ncu_capture_for(key)
         # precision = 1 runs the per-triple work on the FP32 pipe: 128 FFMA lanes per SM, twice the FP64 figure
         peak_nominal = FP64_NOMINAL_TFLOPS * (2.0 if args.precision == 1 else 1.0)
@@ -428,7 +448,8 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_eval": ms_per_step / B,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 0 else "f32 interpolation / f64 geometry+sums", "data": "synthetic",
-                "config": {"workload": desc + (" -- NOTE: BASELINE.json states a batch of 1024 for this config; this run uses "
+                "config": {"emission": cfg["emission"], "interp_domain": cfg["interp_domain"], "phase_interp": cfg["phase_interp"],
+                           "workload": desc + (" -- NOTE: BASELINE.json states a batch of 1024 for this config; this run uses "
                                                "%d per GPU (per-evaluation figure; run --batch 1024 for the stated batch)" % B
                                                if args.workload == "C5" and B != 1024 else ""), "name": args.workload, "precision": args.precision, "tmap_dex": args.tmap, "batch_per_gpu": B, "sub_batch": ctx.sub_batch(), "n_fp": ctx.n_fp,
                            "l2": "flushed before every step (256 MiB write between the steps' CUDA-event brackets)",

@@ -18,6 +18,7 @@
 #include "ppm_geodesic.cuh"
 #include "ppm_cells.cuh"
 #include "ppm_cells32.cuh"
+#include "ppm_cells_lin.cuh"
 #include "ppm_cells_map.cuh"
 #include "ppm_observe.cuh"
 
@@ -243,7 +244,9 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
         "HEALPix mesh: n_phi = 4 N_side and n_theta = 4 N_side - 1");
     ARG(cfg->scratch_mb >= 0, "scratch_mb must be >= 0");
     ARG(cfg->phase_interp == 0 || cfg->phase_interp == 1 || cfg->phase_interp == 3, "phase_interp must be 0 / 1 (linear) or 3");
-    ARG(cfg->interp_domain == 0, "interp_domain must be 0 (log10 I/T^3)");
+    ARG(cfg->interp_domain == 0 || cfg->interp_domain == 1, "interp_domain must be 0 (log10 I/T^3) or 1 (I/T^3)");
+    ARG(cfg->interp_domain == 0 || (cfg->emission != PPM_EMISSION_BLACKBODY && cfg->precision == 0),
+        "interp_domain = 1 applies to table emission with precision = 0");
     for (int e = 0; e < cfg->n_energy; ++e) {
         ARG(std::isfinite(energies[e]) && energies[e] > 0.0, "energies must be finite and > 0");
         if (e) ARG(energies[e] > energies[e - 1], "energies must be strictly increasing");
@@ -464,8 +467,21 @@ static int dispatch_cells_tab32(ppm_ctx* c, const CellArgs& a, dim3 grid, int th
 }
 
 template <int EPL>
+static int dispatch_cells_lin(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    switch (c->npl) {
+    case 1:  return launch_cells(c, k_cells_lin<EPL, 1>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_lin<EPL, 3>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_lin<EPL, 5>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_lin<EPL, 7>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_lin<EPL, 9>, a, grid, threads, smem);
+    }
+}
+
+template <int EPL>
 static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
+    if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
     if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
     switch (c->npl) {
     case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
@@ -548,7 +564,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     if (table && !tmap_dev) {
         SliceArgs S;
         S.spots = c->d_spots; S.rows = c->d_rows; S.values = c->d_values; S.slices = c->d_slices;
-        S.n_theta = g.n_theta; S.nT = c->nT; S.ng = c->ng; S.nmu = c->nmu; S.nx = c->nx;
+        S.n_theta = g.n_theta; S.nT = c->nT; S.ng = c->ng; S.nmu = c->nmu; S.nx = c->nx; S.domain = g.interp_domain;
         dim3 sg((c->nmu * c->nx + 255) / 256, rows);
         prof_begin(c, KID_SLICE);
         k_slice<<<sg, 256, 0, c->stream>>>(S);
@@ -563,8 +579,10 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;
     A.n_fp = c->n_fp; A.nE = g.n_energy;
     A.nmu = table ? c->nmu : 0; A.nx = table ? c->nx : 0;
-    A.mu_rule = g.emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
-    A.x_linedge = g.emission == PPM_EMISSION_TABLE_CUBIC ? 0 : 1;
+    const bool cubic_all = g.emission == PPM_EMISSION_TABLE_CUBIC || g.emission == PPM_EMISSION_TABLE_CUBIC_CLIP;   // a, b
+    A.mu_rule = cubic_all ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
+    A.x_linedge = cubic_all ? 0 : 1;
+    A.clip = (g.interp_domain == 1 && g.emission == PPM_EMISSION_TABLE_CUBIC_CLIP) ? 1 : 0;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh; A.beaming = g.beaming;
     A.phase_order = g.phase_interp == 3 ? 3 : 1; A.y_lo = c->y_lo; A.y_hi = c->y_hi;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
@@ -663,8 +681,8 @@ extern "C" int ppm_evaluate_map(ppm_ctx* c, const double* params_dev, const doub
     if (B == 0) return PPM_OK;
     ARG(params_dev && logT_map_dev && flux_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
-    if (c->cfg.emission != PPM_EMISSION_TABLE_MIXED || c->cfg.precision != 0) {
-        set_err("temperature maps need emission = 2 (linear in log T) and precision = 0"); return PPM_ERR_STATE;
+    if (c->cfg.emission != PPM_EMISSION_TABLE_MIXED || c->cfg.precision != 0 || c->cfg.interp_domain != 0) {
+        set_err("temperature maps need emission = 2 (linear in log T), precision = 0 and interp_domain = 0"); return PPM_ERR_STATE;
     }
     if (!c->have_atm) { set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE; }
     if (c->nT > 64) { set_err("temperature maps support at most 64 log T nodes"); return PPM_ERR_STATE; }

@@ -29,6 +29,7 @@ struct CellArgs {
     int nmu, nx, mu_rule, x_linedge;
     int nchunk, rows_per_chunk, nw, n_etile, mesh;
     int beaming;             // blackbody only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma')
+    int clip;                // intensity-domain interpolation (k_cells_lin): 1 = strategy b, negative intensities -> 0
     int phase_order;         // Interp of Eq 46: 1 linear (reading R11), 3 four-point Lagrange (reading R11b)
     double y_lo, y_hi;       // bounds of log2(10) * (any interpolated table value): a pair whose log2(F_p T^3) + y_lo
                              // < -900 or + y_hi > 900 takes the range-checked energy loop (exponent add must not wrap)
@@ -38,6 +39,7 @@ struct CellArgs {
 struct SliceArgs {
     const SpotD* spots; const RowD* rows; const double* values; double* slices;
     int n_theta, nT, ng, nmu, nx;
+    int domain;              // 0: weighted sum of the tabulated log10(I/T^3) (reading R13a); 1: of I/T^3 = 10^table (R13g)
 };
 
 __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
@@ -58,7 +60,8 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
         for (int b = 0; b < 4; ++b) {
             const double wb = r.wg[b];
             if (wb == 0.0) continue;
-            v = fma(wa * wb, __ldg(A.values + ((size_t)(sp.bT + a) * A.ng + (r.bg + b)) * plane + i), v);
+            const double node = __ldg(A.values + ((size_t)(sp.bT + a) * A.ng + (r.bg + b)) * plane + i);
+            v = fma(wa * wb, A.domain ? exp10(node) : node, v);
         }
     }
     A.slices[(size_t)rid * plane + i] = v;
@@ -327,6 +330,65 @@ __device__ __forceinline__ void smem_check(const void* p, size_t bytes, const vo
 #define PPM_SMEM_CHECK(p, bytes) ((void)0)
 #endif
 
+// ---- fused pass of a pair: node values -> interval coefficients.  Lane l holds nodes n0 .. n0+NPL-1, n0 = jlo-1 + NPL l;
+// interval c (nodes c, c+1) has window offset c - (jlo-1).  Out-of-table nodes read neighbouring shared memory: they only
+// feed window slots that no energy reads.  Node value = sum_mu v_mu S[mu][node] + qb.  Writes KA[0..KW) = (k0,k1),
+// KA[KW..2KW) = (k2,k3); both __syncwarp's are inside (the previous pair's readers are done / the new coefficients are
+// visible).
+template <int NPL>
+__device__ __forceinline__ void fused_pass(const double* __restrict__ srow, int nx, int jlo, int jhi, int lane, double v0,
+                                           double v1, double v2, double v3, double qb, int x_linedge, double2* KA,
+                                           const double* sm)
+{
+    constexpr int KW = 32 * NPL;
+    const int n0 = jlo - 1 + NPL * lane;
+    const double* sp0 = srow + n0;
+    PPM_SMEM_CHECK(sp0, sizeof(double) * (3 * nx + NPL));
+    (void)sm;
+    double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
+#pragma unroll
+    for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node_value(sp0 + jn, nx, v0, v1, v2, v3, qb);
+    f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
+    if (NPL == 1) {
+        f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
+        f[3] = __shfl_down_sync(0xffffffffu, f[1], 2);
+    } else {
+        f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
+        f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
+    }
+    double2 ka[NPL], kb[NPL];
+#pragma unroll
+    for (int jn = 0; jn < NPL; ++jn) cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
+    if (jlo == 0 || jhi == nx - 2) {      // the window holds the first / last interval of the axis (warp-uniform)
+#pragma unroll
+        for (int jn = 0; jn < NPL; ++jn) {
+            const int c = n0 + jn;
+            if (c != 0 && c != nx - 2) continue;
+            if (x_linedge) {                                        // strategies c, d: linear
+                ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
+                kb[jn] = make_double2(0.0, 0.0);
+            } else {                                                // strategies a, b: stencil shifted inward
+                const int s = (c == 0) ? 0 : nx - 4;
+                double g[4];
+#pragma unroll
+                for (int m = 0; m < 4; ++m) g[m] = node_value(srow + s + m, nx, v0, v1, v2, v3, qb);
+                double k0, k1, k2, k3;
+                cubic_coeffs(g[0], g[1], g[2], g[3], k0, k1, k2, k3);
+                const double d = (double)(c - 1 - s);               // Taylor shift to this interval's midpoint
+                ka[jn] = make_double2(fma(d, fma(d, fma(d, k3, k2), k1), k0), fma(d, fma(3.0 * d, k3, 2.0 * k2), k1));
+                kb[jn] = make_double2(fma(3.0 * d, k3, k2), k3);
+            }
+        }
+    }
+    __syncwarp();                                                   // the previous pair's readers are done
+#pragma unroll
+    for (int jn = 0; jn < NPL; ++jn) {
+        KA[NPL * lane + jn] = ka[jn];
+        KA[NPL * lane + jn + KW] = kb[jn];
+    }
+    __syncwarp();
+}
+
 // one triple: logx coordinate s (fixed point) -> interval coefficients -> y -> 2^y (no range checks)
 template <int KW>
 __device__ __forceinline__ double triple_value(const double2* __restrict__ KAq, long long s)
@@ -503,54 +565,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                 const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
                 const double* srow = S + (inf & 0xFFFF);
-                // ---- fused pass: node values -> interval coefficients.  Lane l holds nodes n0 .. n0+NPL-1, n0 = jlo-1 + NPL l;
-                // interval c (nodes c, c+1) has window offset c - (jlo-1).  Out-of-table nodes read neighbouring shared memory:
-                // they only feed window slots that no energy reads.
-                const int n0 = jlo - 1 + NPL * lane;
-                const double* sp0 = srow + n0;
-                PPM_SMEM_CHECK(sp0, sizeof(double) * (3 * nx + NPL));
-                double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
-#pragma unroll
-                for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node_value(sp0 + jn, nx, v0, v1, v2, v3, qb);
-                f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
-                if (NPL == 1) {
-                    f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
-                    f[3] = __shfl_down_sync(0xffffffffu, f[1], 2);
-                } else {
-                    f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
-                    f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
-                }
-                double2 ka[NPL], kb[NPL];
-#pragma unroll
-                for (int jn = 0; jn < NPL; ++jn) cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
-                if (jlo == 0 || jhi == nx - 2) {      // the window holds the first / last interval of the axis (warp-uniform)
-#pragma unroll
-                    for (int jn = 0; jn < NPL; ++jn) {
-                        const int c = n0 + jn;
-                        if (c != 0 && c != nx - 2) continue;
-                        if (A.x_linedge) {                                      // strategy d: linear
-                            ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
-                            kb[jn] = make_double2(0.0, 0.0);
-                        } else {                                                // strategy a: stencil shifted inward
-                            const int s = (c == 0) ? 0 : nx - 4;
-                            double g[4];
-#pragma unroll
-                            for (int m = 0; m < 4; ++m) g[m] = node_value(srow + s + m, nx, v0, v1, v2, v3, qb);
-                            double k0, k1, k2, k3;
-                            cubic_coeffs(g[0], g[1], g[2], g[3], k0, k1, k2, k3);
-                            const double d = (double)(c - 1 - s);               // Taylor shift to this interval's midpoint
-                            ka[jn] = make_double2(fma(d, fma(d, fma(d, k3, k2), k1), k0), fma(d, fma(3.0 * d, k3, 2.0 * k2), k1));
-                            kb[jn] = make_double2(fma(3.0 * d, k3, k2), k3);
-                        }
-                    }
-                }
-                __syncwarp();                                                   // the previous pair's readers are done
-#pragma unroll
-                for (int jn = 0; jn < NPL; ++jn) {
-                    KA[NPL * lane + jn] = ka[jn];
-                    KA[NPL * lane + jn + KW] = kb[jn];
-                }
-                __syncwarp();
+                fused_pass<NPL>(srow, nx, jlo, jhi, lane, v0, v1, v2, v3, qb, A.x_linedge, KA, sm);
                 const double2* KAq = KA + (1 - jlo);
                 // ---- energies ----
                 if (flg == 0) {
@@ -566,8 +581,10 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                     // their term the pair's constant 2^y(s_top).  Groups g .. EPL-1 (g = flg >> 8) are clamped for every lane:
                     // the constant goes to lane g's deferred sum and is spread over acc[g ..] once, in the epilogue.
                     const int g = flg >> 8;
-                    const double vtop = triple_value<KW>(KAq, s_top);
-                    if (lane == g) hdef += vtop;
+                    if (g < EPL) {                                              // (g == EPL: only the last group straddles the end)
+                        const double vtop = triple_value<KW>(KAq, s_top);
+                        if (lane == g) hdef += vtop;
+                    }
                     dispatch_clamped_hi<KW, EPL, EPL>(g, acc, uef, KAq, q, s_top);
                 } else {
                     // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,

@@ -107,7 +107,7 @@ __device__ inline void cheb_eval(const double* __restrict__ c, double s, double&
 // rule of the log T and log g axes per emission mode (strategies a, d, c; readings R13c, R13e)
 __host__ __device__ inline int tg_rule(int emission)
 {
-    return emission == PPM_EMISSION_TABLE_CUBIC ? AX_CUBIC_SHIFT
+    return (emission == PPM_EMISSION_TABLE_CUBIC || emission == PPM_EMISSION_TABLE_CUBIC_CLIP) ? AX_CUBIC_SHIFT
          : emission == PPM_EMISSION_TABLE_CUBIC_LINEDGE ? AX_CUBIC_LINEDGE : AX_LINEAR;
 }
 
