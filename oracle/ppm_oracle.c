@@ -953,6 +953,115 @@ double orc_chi2(const double* m, const double* d, size_t n)
     return 1.0e6 / sm * s;
 }
 
+/* ------------------------------------------------------------------------------------
+ * O10  Reference chain for the device-resident sampler loop (PAPER.md:716 names "a fully GPU-resident
+ * parallel-tempered MCMC" without giving an algorithm -> reading R26): W walkers, walker w at inverse temperature
+ * beta[w]; per step (i) Gaussian random-walk proposal p' = p + sigma * n inside a box prior [lo, hi] (outside: rejected),
+ * (ii) Metropolis accept iff ln u < beta_w (lnL' - lnL), (iii) replica exchange between the neighbours (i, i+1) with
+ * i = t mod 2, t mod 2 + 2, ...: swap iff ln u < (beta_i - beta_{i+1}) (lnL_{i+1} - lnL_i).
+ * All random numbers come from the counter-based generator Philox4x32-10 (Salmon et al. 2011) keyed by the seed, with the
+ * counter (t low, t high, walker, stream): streams 0..P/2 -> proposal normals of parameters (2 s, 2 s + 1) by Box-Muller,
+ * 0x10000 -> accept uniform, 0x10001 -> swap uniform of the pair starting at `walker`.
+ * ---------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* 53-bit uniform in (0, 1) from two 32-bit words */
+static double u01(uint32_t a, uint32_t b)
+{
+    uint64_t m = ((uint64_t)(a >> 5) << 26) | (uint64_t)(b >> 6);
+    return ((double)m + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+/* two uniforms (u0, u1) and the two Box-Muller normals (n0, n1) of counter (t, walker, stream) */
+void orc_chain_random(uint64_t seed, uint64_t t, uint32_t walker, uint32_t stream, double* u0, double* u1, double* n0, double* n1)
+{
+    uint32_t ctr[4] = { (uint32_t)t, (uint32_t)(t >> 32), walker, stream };
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
+    orc_philox4x32_10(ctr, key, x);
+    double a = u01(x[0], x[1]), b = u01(x[2], x[3]);
+    double r = sqrt(-2.0 * log(a));
+    *u0 = a; *u1 = b; *n0 = r * cos(2.0 * M_PI * b); *n1 = r * sin(2.0 * M_PI * b);
+}
+
+/* ln L of one parameter vector: O2-O9 in sequence (evaluate, fold, Poisson likelihood); -inf outside the model's domain */
+static double chain_loglike(const orc_config* cfg, const double* energies, const orc_atm* atm, const double* p,
+                            int n_channel, int band_w, const int32_t* first_chan, const double* rsp_band,
+                            const double* tau_ref, const double* data, const double* bkg, double exposure_s,
+                            double* flux, double* counts)
+{
+    if (orc_evaluate(cfg, energies, p, atm, NULL, 0, flux, NULL) != 0) return -INFINITY;
+    orc_fold(flux, cfg->n_phase, cfg->n_energy, n_channel, band_w, first_chan, rsp_band, tau_ref, p[5], counts);
+    return orc_loglike(counts, data, bkg, cfg->n_phase, n_channel, exposure_s);
+}
+
+/* Runs n_steps of the chain in place.  params [W][P], loglike [W] (in: ln L of params; out: updated), accepted [W],
+ * swapped [W] (exchanges that moved a new state into slot w).  t0 = index of the first step.  margin (optional): the
+ * smallest |ln u - log acceptance ratio| met, so that a test can tell a robust decision from a coin flip. */
+void orc_chain_run(const orc_config* cfg, const double* energies, const orc_atm* atm, int n_channel, int band_w,
+                   const int32_t* first_chan, const double* rsp_band, const double* tau_ref, const double* data,
+                   const double* bkg, double exposure_s, int W, const double* lo, const double* hi, const double* sigma,
+                   const double* beta, uint64_t seed, uint64_t t0, int n_steps, double* params, double* loglike,
+                   int64_t* accepted, int64_t* swapped, double* margin)
+{
+    const int P = 8 + 8 * cfg->n_spots;
+    double* prop = (double*)malloc(sizeof(double) * P);
+    double* flux = (double*)malloc(sizeof(double) * (size_t)cfg->n_phase * cfg->n_energy);
+    double* counts = (double*)malloc(sizeof(double) * (size_t)cfg->n_phase * n_channel);
+    double mg = INFINITY;
+    for (int st = 0; st < n_steps; ++st) {
+        const uint64_t t = t0 + (uint64_t)st;
+        for (int w = 0; w < W; ++w) {
+            double* cur = params + (size_t)w * P;
+            int inside = 1;
+            for (int k = 0; k < P; ++k) {
+                prop[k] = cur[k];
+                if (sigma[k] > 0.0) {
+                    double u0, u1, n0, n1;
+                    orc_chain_random(seed, t, (uint32_t)w, (uint32_t)(k / 2), &u0, &u1, &n0, &n1);
+                    prop[k] = cur[k] + sigma[k] * ((k & 1) ? n1 : n0);
+                    if (!(prop[k] >= lo[k] && prop[k] <= hi[k])) inside = 0;
+                }
+            }
+            if (!inside) continue;                                       /* zero prior: rejected without evaluation */
+            double lp = chain_loglike(cfg, energies, atm, prop, n_channel, band_w, first_chan, rsp_band, tau_ref, data, bkg,
+                                      exposure_s, flux, counts);
+            double u0, u1, n0, n1;
+            orc_chain_random(seed, t, (uint32_t)w, 0x10000u, &u0, &u1, &n0, &n1);
+            double ratio = beta[w] * (lp - loglike[w]);
+            if (isfinite(lp) && fabs(log(u0) - ratio) < mg) mg = fabs(log(u0) - ratio);
+            if (isfinite(lp) && log(u0) < ratio) {
+                memcpy(cur, prop, sizeof(double) * P);
+                loglike[w] = lp;
+                accepted[w] += 1;
+            }
+        }
+        for (int i = (int)(t & 1); i + 1 < W; i += 2) {                  /* replica exchange, reading R26 (iii) */
+            double u0, u1, n0, n1;
+            orc_chain_random(seed, t, (uint32_t)i, 0x10001u, &u0, &u1, &n0, &n1);
+            double ratio = (beta[i] - beta[i + 1]) * (loglike[i + 1] - loglike[i]);
+            if (beta[i] != beta[i + 1] && fabs(log(u0) - ratio) < mg) mg = fabs(log(u0) - ratio);
+            if (log(u0) < ratio) {
+                for (int k = 0; k < P; ++k) { double x = params[(size_t)i * P + k]; params[(size_t)i * P + k] = params[(size_t)(i + 1) * P + k]; params[(size_t)(i + 1) * P + k] = x; }
+                double x = loglike[i]; loglike[i] = loglike[i + 1]; loglike[i + 1] = x;
+                swapped[i] += 1; swapped[i + 1] += 1;
+            }
+        }
+    }
+    if (margin) *margin = mg;
+    free(prop); free(flux); free(counts);
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

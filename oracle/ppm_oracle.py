@@ -88,6 +88,13 @@ _hp_ring = _sig("orc_healpix_ring", None, [C.c_int, C.c_int, _dp, C.POINTER(C.c_
 _hp_mask = _sig("orc_spot_mask_healpix", C.c_int, [C.POINTER(Spot), C.c_int, _u8p])
 _hp_row = _sig("orc_row_init_healpix", None, [C.POINTER(Star), C.c_int, C.c_int, C.POINTER(Row)])
 _chi2 = _sig("orc_chi2", C.c_double, [_dp, _dp, C.c_size_t])
+_u32p = C.POINTER(C.c_uint32)
+_i64p = C.POINTER(C.c_int64)
+_philox = _sig("orc_philox4x32_10", None, [_u32p, _u32p, _u32p])
+_chain_random = _sig("orc_chain_random", None, [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _dp, _dp, _dp, _dp])
+_chain_run = _sig("orc_chain_run", None,
+                  [C.POINTER(_Config), _dp, C.POINTER(_Atm), C.c_int, C.c_int, _ip, _dp, _dp, _dp, _dp, C.c_double, C.c_int,
+                   _dp, _dp, _dp, _dp, C.c_uint64, C.c_uint64, C.c_int, _dp, _dp, _i64p, _i64p, _dp])
 _nthreads = _sig("orc_num_threads", C.c_int, [])
 _set_nthreads = _sig("orc_set_num_threads", None, [C.c_int])
 
@@ -315,6 +322,44 @@ def loglike(counts, data, bkg, exposure_s):
 def chi2(m, d):
     m, d = _f64(m).ravel(), _f64(d).ravel()
     return _chi2(_p(m), _p(d), m.size)
+
+
+def philox4x32_10(ctr, key):
+    c = np.ascontiguousarray(ctr, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    _philox(c.ctypes.data_as(_u32p), k.ctypes.data_as(_u32p), out.ctypes.data_as(_u32p))
+    return out
+
+
+def chain_random(seed, t, walker, stream):
+    """-> (u0, u1, n0, n1) of counter (t, walker, stream) under key `seed` (reading R26)."""
+    v = [C.c_double() for _ in range(4)]
+    _chain_random(int(seed), int(t), int(walker), int(stream), *[C.byref(x) for x in v])
+    return tuple(x.value for x in v)
+
+
+def chain_run(cfg, energies, atm, rsp, data, bkg, exposure_s, params, loglike, lo, hi, sigma, beta, seed, t0, n_steps):
+    """Reference sampler loop (O10).  params [W][P] and loglike [W] are updated in place.
+    -> (accepted [W], swapped [W], margin)."""
+    energies = _f64(energies)
+    c = _Config(cfg["n_spots"], cfg["n_theta"], cfg["n_phi"], cfg["n_phase"], cfg["n_fp"], len(energies), cfg["emission"],
+                int(cfg.get("oblate", 1)), int(cfg.get("mesh", 0)), int(cfg.get("beaming", 0)),
+                int(cfg.get("phase_interp", 0)), int(cfg.get("interp_domain", 0)))
+    assert params.dtype == np.float64 and params.flags.c_contiguous and loglike.dtype == np.float64
+    W = params.shape[0]
+    fc = np.ascontiguousarray(rsp["first_chan"], dtype=np.int32)
+    band, tau = _f64(rsp["rsp_band"]), _f64(rsp["tau_ref"])
+    data, bkg = _f64(data), _f64(bkg)
+    lo, hi, sigma, beta = _f64(lo), _f64(hi), _f64(sigma), _f64(beta)
+    acc = np.zeros(W, dtype=np.int64)
+    swp = np.zeros(W, dtype=np.int64)
+    mg = C.c_double()
+    _chain_run(C.byref(c), _p(energies), C.byref(atm.c) if atm is not None else None, int(rsp["n_channel"]), band.shape[1],
+               fc.ctypes.data_as(_ip), _p(band), _p(tau), _p(data), _p(bkg), float(exposure_s), W, _p(lo), _p(hi), _p(sigma),
+               _p(beta), int(seed), int(t0), int(n_steps), _p(params), _p(loglike), acc.ctypes.data_as(_i64p),
+               swp.ctypes.data_as(_i64p), C.byref(mg))
+    return acc, swp, mg.value
 
 
 def num_threads():
