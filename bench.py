@@ -270,6 +270,10 @@ def main():
                     help="override the workload's interpolation strategy: 1 a, 4 b, 3 c, 2 d (PAPER.md:551)")
     ap.add_argument("--interp-domain", type=int, default=0, choices=[0, 1],
                     help="1: the table interpolation acts on I/T^3 instead of its logarithm (reading R13g)")
+    ap.add_argument("--chain", action="store_true",
+                    help="time the device-resident sampler loop (ppm_chain_run: proposal kernel -> S0-S7 -> accept -> exchange, one "
+                         "CUDA-graph replay per step, --batch walkers); e2e is then the same Metropolis step driven from the host "
+                         "through ppm_loglike_host")
     ap.add_argument("--phase-interp", type=int, default=0, choices=[0, 1, 3], help="order of Interp in Eq 46 (reading R11b)")
     ap.add_argument("--batch", type=int, default=8,
                     help="parameter vectors per GPU and step (C5: BASELINE.json states 1024; the default 8 gives the "
@@ -341,7 +345,38 @@ def main():
         ctx.fold_response(flux, params, counts)
         ctx.loglike(counts, data, bkg, exposure, ll)
 
+    chain_box = None
+    if args.chain:
+        P = conf["params"].shape[1]
+        lo, hi, sig = np.full(P, -1e30), np.full(P, 1e30), np.zeros(P)
+        for k0, (a, b_, s_) in {0: (1.0, 3.0, 0.01), 1: (8.0, 16.0, 0.05), 3: (0.0, 1.0, 0.005), 5: (0.05, 3.0, 0.01)}.items():
+            lo[k0], hi[k0], sig[k0] = a, b_, s_
+        for sp_ in range(cfg["n_spots"]):
+            for off, (a, b_, s_) in {0: (0.1, np.pi - 0.1, 0.005), 2: (0.05, 1.0, 0.005), 3: (5.6, 6.5, 0.002)}.items():
+                lo[8 + 8 * sp_ + off], hi[8 + 8 * sp_ + off], sig[8 + 8 * sp_ + off] = a, b_, s_
+        chain_box = (lo, hi, sig)
+        ctx.chain_create(conf["params"], lo, hi, sig, data, bkg, exposure, seed=gen.SEED0)
+        host_state = {"p": conf["params"].copy(), "ll": None, "rng": np.random.default_rng(gen.SEED0)}
+
+    def step_chain():
+        ctx.chain_run(1)
+
+    def step_chain_host():
+        """the same Metropolis step driven from the host: proposals and acceptance in numpy, ln L through ppm_loglike_host"""
+        lo, hi, sig = chain_box
+        if host_state["ll"] is None:
+            host_state["ll"] = ctx.loglike_host(host_state["p"], data, bkg, exposure)[0].copy()
+        prop = host_state["p"] + sig[None, :] * host_state["rng"].standard_normal(host_state["p"].shape)
+        inside = np.all((prop >= lo) & (prop <= hi) | (sig == 0), axis=1)
+        prop[~inside] = host_state["p"][~inside]
+        llp, _ = ctx.loglike_host(prop, data, bkg, exposure)
+        acc = inside & np.isfinite(llp) & (np.log(host_state["rng"].uniform(size=len(llp))) < llp - host_state["ll"])
+        host_state["p"][acc] = prop[acc]
+        host_state["ll"][acc] = llp[acc]
+
     def step_e2e():
+        if args.chain:
+            return step_chain_host()
         if tmap is not None:               # no host-buffer entry for maps: device-pointer calls + explicit copies
             params.copy_(params_pinned, non_blocking=True)
             step()
@@ -380,18 +415,24 @@ def main():
     n0 = ctx.launch_count()
     ctx.profile_enable(True)
     t_begin = time.time()
-    total_ms, wall_ms, per = timed(step, args.steps)
+    if args.chain:
+        for _ in range(args.warmup):
+            step_chain()
+        n0 = ctx.launch_count()
+    total_ms, wall_ms, per = timed(step_chain if args.chain else step, args.steps)
     clk = clocks.stop(t_begin, time.time())
+    launches = ctx.launch_count() - n0
+    if args.chain:                              # the captured step holds no event records: per-kernel times from eager steps
+        timed(step, args.steps)
     prof, triples = ctx.profile_read()
     ctx.profile_enable(False)
-    launches = ctx.launch_count() - n0
     ll_dev = ll.cpu().numpy().copy()
 
     # e2e: host buffers through the C ABI, copies inside the timed region
     for _ in range(2):
         step_e2e()
     e2e_total, _, _ = timed(step_e2e, args.steps)
-    assert np.array_equal(ll_host, ll_dev), "host-buffer path must reproduce the device-pointer path bit for bit"
+    assert args.chain or np.array_equal(ll_host, ll_dev), "host-buffer path must reproduce the device-pointer path bit for bit"
 
     ms_per_step = total_ms / args.steps
     value = world * B * args.steps / (total_ms * 1e-3)
@@ -453,10 +494,12 @@ def main():
                                                "%d per GPU (per-evaluation figure; run --batch 1024 for the stated batch)" % B
                                                if args.workload == "C5" and B != 1024 else ""), "name": args.workload, "precision": args.precision, "tmap_dex": args.tmap, "batch_per_gpu": B, "sub_batch": ctx.sub_batch(), "n_fp": ctx.n_fp,
                            "l2": "flushed before every step (256 MiB write between the steps' CUDA-event brackets)",
-                           "step": "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
+                           "step": ("ppm_chain_run(1): proposal kernel + S0-S7 + accept + exchange, one CUDA-graph replay, %d walkers" % B)
+                                   if args.chain else "ppm_evaluate + ppm_fold_response + ppm_loglike (S0-S7)"},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params_pinned.numel() * 8),
                         "d2h_bytes_per_step": int(ll_host.nbytes + st_host.nbytes),
-                        "call": "ppm_loglike_host (host params in, host ln L + status out)"},
+                        "call": "host-driven Metropolis step: numpy proposals + ppm_loglike_host + numpy acceptance" if args.chain
+                                else "ppm_loglike_host (host params in, host ln L + status out)"},
                 "gpu_launches": int(launches), "clocks": clk, "wall_ms_per_step": wall_ms / args.steps,
                 "step_ms": [round(x, 3) for x in per], "roofline": roofline, "cpu_baseline": None}
         if world == 1 and not args.no_cpu_baseline:

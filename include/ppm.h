@@ -148,6 +148,26 @@ int ppm_loglike_host(ppm_ctx* ctx, const double* params_host, int B, const doubl
                      const double* bkg_dev, double exposure_s, double* loglike_host,
                      int32_t* status_host);
 
+/* Device-resident sampler loop around the likelihood (reading R26 of DESIGN.md).
+ * ppm_chain_create: W = n_walkers <= max_batch walkers start at params0_host [W][P]; parameter k is proposed as
+ *   p_k + sigma_host[k] * N(0,1) (sigma 0 = fixed) inside the box prior [lo_host[k], hi_host[k]] (outside: rejected);
+ *   walker w has inverse temperature beta_host[w] (NULL = all 1); data_dev [n_phase][n_channel], bkg_dev [n_channel] or
+ *   NULL and exposure_s as in ppm_loglike (the data buffers must stay valid while the chain lives).  Needs a response
+ *   (ppm_set_response) and, for table emission, an atmosphere.  Evaluates ln L of the starting states; synchronises.
+ * ppm_chain_run: n_steps steps, each = proposal kernel -> S0..S7 (ppm_evaluate + ppm_fold_response + ppm_loglike on the
+ *   proposals, in HBM) -> Metropolis acceptance against beta_w (ln L' - ln L) -> replica exchange between neighbouring
+ *   walkers.  The step is captured into a CUDA graph at the first call and replayed; asynchronous on the context's stream.
+ *   Random numbers: Philox4x32-10, key = seed, counter = (step, walker, stream).
+ * ppm_chain_read: synchronises and copies the current states [W][P], their ln L [W], the per-walker counts of accepted
+ *   proposals and exchanges [W] and the number of steps done (any pointer may be NULL).
+ * One chain per context; ppm_chain_create on a context that has one replaces it; ppm_destroy frees it. */
+int ppm_chain_create(ppm_ctx* ctx, int n_walkers, const double* params0_host, const double* lo_host,
+                     const double* hi_host, const double* sigma_host, const double* beta_host, uint64_t seed,
+                     const double* data_dev, const double* bkg_dev, double exposure_s);
+int ppm_chain_run(ppm_ctx* ctx, int n_steps);
+int ppm_chain_read(ppm_ctx* ctx, double* params_host, double* loglike_host, int64_t* accepted_host,
+                   int64_t* swapped_host, int64_t* steps_host);
+
 /* Introspection of the intermediate device state left by the LAST ppm_evaluate call, for
  * vector b of that call (tests compare each step with the oracle).  All outputs are host
  * buffers; row index r = spot * n_theta + j.

@@ -39,6 +39,9 @@ EXPORTS = {
     "ppm_loglike": (C.c_int, [_vp, _vp, C.c_int, _vp, _vp, C.c_double, _vp]),
     "ppm_evaluate_host": (C.c_int, [_vp, _dp, C.c_int, _dp, _ip]),
     "ppm_loglike_host": (C.c_int, [_vp, _dp, C.c_int, _vp, _vp, C.c_double, _dp, _ip]),
+    "ppm_chain_create": (C.c_int, [_vp, C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_uint64, _vp, _vp, C.c_double]),
+    "ppm_chain_run": (C.c_int, [_vp, C.c_int]),
+    "ppm_chain_read": (C.c_int, [_vp, _dp, _dp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
     "ppm_debug_rows": (C.c_int, [_vp, C.c_int, _dp]),
     "ppm_debug_mask": (C.c_int, [_vp, C.c_int, _u8p]),
     "ppm_debug_template": (C.c_int, [_vp, C.c_int, _dp]),
@@ -270,6 +273,37 @@ class PPM:
         _check(self.lib.ppm_loglike_host(self._h, _np(params), B, _dev(data, t.float64, "data", (self.n_phase, self.n_channel)), bp, float(exposure_s),
                                          _np(out), status.ctypes.data_as(_ip)))
         return out, status
+
+    # ---- device-resident sampler loop ----
+    def chain_create(self, params0, lo, hi, sigma, data, bkg, exposure_s, beta=None, seed=0):
+        t = self.torch
+        self._on_stream()
+        params0 = _f64(params0).reshape(-1, self.P)
+        W = params0.shape[0]
+        lo, hi, sigma = (_host(_f64(a), np.float64, (self.P,), n) for a, n in ((lo, "lo"), (hi, "hi"), (sigma, "sigma")))
+        bp = None
+        if beta is not None:
+            beta = _host(_f64(beta), np.float64, (W,), "beta")
+            bp = _np(beta)
+        bk = _dev(bkg, t.float64, "bkg", (self.n_channel,)) if bkg is not None else C.c_void_p(0)
+        self._chain_keep = (data, bkg)                       # the chain reads these device buffers at every step
+        _check(self.lib.ppm_chain_create(self._h, W, _np(params0), _np(lo), _np(hi), _np(sigma), bp, int(seed),
+                                         _dev(data, t.float64, "data", (self.n_phase, self.n_channel)), bk, float(exposure_s)))
+        self._chain_w = W
+
+    def chain_run(self, n_steps):
+        self._on_stream()
+        _check(self.lib.ppm_chain_run(self._h, int(n_steps)))
+
+    def chain_read(self):
+        """-> (params [W][P], loglike [W], accepted [W], swapped [W], steps)"""
+        W = self._chain_w
+        p, ll = np.empty((W, self.P)), np.empty(W)
+        acc, swp = np.zeros(W, dtype=np.int64), np.zeros(W, dtype=np.int64)
+        st = C.c_int64()
+        i64 = C.POINTER(C.c_int64)
+        _check(self.lib.ppm_chain_read(self._h, _np(p), _np(ll), acc.ctypes.data_as(i64), swp.ctypes.data_as(i64), C.byref(st)))
+        return p, ll, acc, swp, st.value
 
     # ---- introspection of the last evaluate (tests) ----
     def debug_rows(self, b=0):

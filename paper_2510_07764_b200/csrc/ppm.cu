@@ -21,6 +21,7 @@
 #include "ppm_cells_lin.cuh"
 #include "ppm_cells_map.cuh"
 #include "ppm_observe.cuh"
+#include "ppm_chain.cuh"
 
 using namespace ppm;
 
@@ -110,6 +111,7 @@ struct ppm_ctx {
     double* d_en = nullptr;
     long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
     int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
+    int chunk = 1;                                // consecutive energies per lane chunk of k_cells_tab (1 = strided ownership)
     std::vector<double> h_en;
     // atmosphere
     bool have_atm = false;
@@ -136,6 +138,16 @@ struct ppm_ctx {
     std::vector<int> prof_kid;                    // kernel id of each recorded launch
     size_t prof_used = 0;
     unsigned long long* d_pairs = nullptr;        // (cell, phase) pairs with F_p != 0 walked by k_cells
+    // device-resident sampler loop (ppm_chain_*)
+    ChainArgs chain{};
+    double* d_chain_box = nullptr;                // lo | hi | sigma [3][P]
+    double* d_chain_beta = nullptr;
+    const double *chain_data = nullptr, *chain_bkg = nullptr;
+    double chain_exposure = 0.0;
+    cudaGraphExec_t chain_graph = nullptr;
+    int64_t chain_launches_per_step = 0;
+    cudaStream_t chain_stream = nullptr;          // own stream when the context runs on the legacy default stream (which
+    cudaEvent_t chain_ev = nullptr;               // cannot be captured); ordered with it through chain_ev
 };
 
 // kernel ids of ppm_profile_read
@@ -161,10 +173,23 @@ static void prof_end(ppm_ctx* c)
 
 extern "C" const char* ppm_last_error(void) { return g_err; }
 
+static void chain_free(ppm_ctx* c)
+{
+    if (c->chain_graph) { cudaGraphExecDestroy(c->chain_graph); c->chain_graph = nullptr; }
+    if (c->chain_stream) { cudaStreamSynchronize(c->chain_stream); cudaStreamDestroy(c->chain_stream); c->chain_stream = nullptr; }
+    if (c->chain_ev) { cudaEventDestroy(c->chain_ev); c->chain_ev = nullptr; }
+    void* ptrs[] = {c->chain.cur, c->chain.prop, c->chain.ll, c->chain.llp, c->chain.oob, c->chain.accepted, c->chain.swapped,
+                    c->chain.t, c->d_chain_box, c->d_chain_beta};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    c->chain = ChainArgs{};
+    c->d_chain_box = nullptr; c->d_chain_beta = nullptr;
+}
+
 extern "C" int ppm_destroy(ppm_ctx* c)
 {
     if (!c) return PPM_OK;
     cudaSetDevice(c->cfg.device);
+    chain_free(c);
     void* ptrs[] = {c->d_en, c->d_uef, c->d_axT, c->d_axg, c->d_axmu, c->d_values, c->d_first, c->d_elo,
                     c->d_ehi, c->d_band, c->d_tau, c->d_stars, c->d_spots, c->d_rows, c->d_cells, c->d_lookup,
                     c->d_tmpl, c->d_slices, c->d_partial, c->d_params_stage, c->d_flux_stage,
@@ -203,6 +228,7 @@ static int compute_sb(const ppm_ctx* c, size_t slice_doubles)
 
 static void free_scratch(ppm_ctx* c)
 {
+    if (c->chain_graph) { cudaGraphExecDestroy(c->chain_graph); c->chain_graph = nullptr; }   // captured pointers go stale
     void** ptrs[] = {(void**)&c->d_stars, (void**)&c->d_spots, (void**)&c->d_rows, (void**)&c->d_cells, (void**)&c->d_lookup,
                      (void**)&c->d_tmpl, (void**)&c->d_partial, (void**)&c->d_pairs, (void**)&c->d_slices,
                      (void**)&c->d_flux_stage, (void**)&c->d_counts_stage};
@@ -402,6 +428,25 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
             return PPM_ERR_ARG;
         }
     }
+    // Chunked energy ownership of k_cells_tab (ppm_cells.cuh): CH consecutive energies per lane chunk share two coefficient
+    // records when every chunk spans less than one logx interval.  Instantiated for the dense-grid shapes (EPL 10 / 8, NPL 3).
+    c->chunk = 1;
+    if (c->cfg.precision == 0 && c->cfg.interp_domain == 0 && c->npl == 3 && (c->epl == 10 || c->epl == 8)) {
+        const int nE = c->cfg.n_energy, epl = c->epl;
+        for (int ch : {4, 3}) {
+            bool ok = true;
+            for (int t = 0; t < c->n_etile && ok; ++t)
+                for (int cc = 0; cc * ch < epl && ok; ++cc) {
+                    const int ncc = std::min(ch, epl - ch * cc);
+                    for (int lane = 0; lane < 32 && ok; ++lane) {
+                        const int ea = t * 32 * epl + 32 * ch * cc + ncc * lane, eb = ea + ncc - 1;
+                        if (ea >= nE) continue;
+                        ok = uef[std::min(eb, nE - 1)] - uef[ea] < (1ll << 52) - 4;
+                    }
+                }
+            if (ok) { c->chunk = ch; break; }
+        }
+    }
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;
@@ -483,6 +528,10 @@ static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int thre
 {
     if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
     if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
+    if constexpr (EPL == 10 || EPL == 8) {
+        if (c->npl == 3 && c->chunk == 4) return launch_cells(c, k_cells_tab<EPL, 3, 4>, a, grid, threads, smem);
+        if (c->npl == 3 && c->chunk == 3) return launch_cells(c, k_cells_tab<EPL, 3, 3>, a, grid, threads, smem);
+    }
     switch (c->npl) {
     case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
     case 3:  return launch_cells(c, k_cells_tab<EPL, 3>, a, grid, threads, smem);
@@ -837,6 +886,145 @@ extern "C" int ppm_loglike_host(ppm_ctx* c, const double* params_host, int B, co
     if (status_host)
         CK(cudaMemcpyAsync(status_host, c->d_status_stage, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
+    return PPM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// device-resident sampler loop (ppm_chain.cuh)
+// ------------------------------------------------------------------------------------------------
+// ln L of `n` parameter vectors that sit in device memory, into ll_dev: S0..S7 in sub-batches, nothing leaves the device
+static int loglike_resident(ppm_ctx* c, const double* params_dev, int n, double* ll_dev)
+{
+    for (int b0 = 0; b0 < n; b0 += c->SB) {
+        const int nb = std::min(c->SB, n - b0);
+        const double* pd = params_dev + (size_t)b0 * c->P;
+        int rc;
+        if ((rc = evaluate_sub(c, pd, nb, c->d_flux_stage, c->d_status_stage + b0))) return rc;
+        if ((rc = ppm_fold_response(c, c->d_flux_stage, pd, nb, c->d_counts_stage))) return rc;
+        if ((rc = ppm_loglike(c, c->d_counts_stage, nb, c->chain_data, c->chain_bkg, c->chain_exposure, ll_dev + b0))) return rc;
+    }
+    return PPM_OK;
+}
+
+extern "C" int ppm_chain_create(ppm_ctx* c, int W, const double* params0, const double* lo, const double* hi,
+                                const double* sigma, const double* beta, uint64_t seed, const double* data_dev,
+                                const double* bkg_dev, double exposure_s)
+{
+    ARG(c, "null context");
+    ARG(params0 && lo && hi && sigma && data_dev, "null pointer");
+    ARG(W >= 1 && W <= c->cfg.max_batch, "n_walkers must be in 1 .. max_batch");
+    if (!c->have_rsp) { set_err("no response set"); return PPM_ERR_STATE; }
+    if (c->cfg.emission != PPM_EMISSION_BLACKBODY && !c->have_atm) {
+        set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE;
+    }
+    const int P = c->P;
+    for (int k = 0; k < P; ++k) ARG(sigma[k] >= 0.0 && (sigma[k] == 0.0 || lo[k] <= hi[k]), "sigma must be >= 0 and lo <= hi");
+    CK(cudaSetDevice(c->cfg.device));
+    CK(cudaStreamSynchronize(c->stream));
+    chain_free(c);
+    int rc = ensure_stage(c);
+    if (rc) return rc;
+    const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy, cstride = (size_t)c->cfg.n_phase * c->n_channel;
+    if (!c->d_flux_stage && (rc = dev_alloc(&c->d_flux_stage, (size_t)c->SB * fstride))) return rc;
+    if (!c->d_counts_stage && (rc = dev_alloc(&c->d_counts_stage, (size_t)c->SB * cstride))) return rc;
+    ChainArgs& A = c->chain;
+    if ((rc = dev_alloc(&A.cur, (size_t)W * P)) || (rc = dev_alloc(&A.prop, (size_t)W * P)) || (rc = dev_alloc(&A.ll, (size_t)W)) ||
+        (rc = dev_alloc(&A.llp, (size_t)W)) || (rc = dev_alloc(&A.oob, (size_t)W)) || (rc = dev_alloc(&A.accepted, (size_t)W)) ||
+        (rc = dev_alloc(&A.swapped, (size_t)W)) || (rc = dev_alloc(&A.t, (size_t)1)) ||
+        (rc = dev_alloc(&c->d_chain_box, (size_t)3 * P)) || (rc = dev_alloc(&c->d_chain_beta, (size_t)W))) {
+        chain_free(c);
+        return rc;
+    }
+    std::vector<double> bt(W, 1.0);
+    if (beta) bt.assign(beta, beta + W);
+    cudaError_t e = cudaMemcpyAsync(A.cur, params0, sizeof(double) * W * P, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_chain_box, lo, sizeof(double) * P, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_chain_box + P, hi, sizeof(double) * P, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_chain_box + 2 * P, sigma, sizeof(double) * P, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_chain_beta, bt.data(), sizeof(double) * W, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A.accepted, 0, sizeof(long long) * W, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A.swapped, 0, sizeof(long long) * W, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A.t, 0, sizeof(unsigned long long), c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(A.oob, 0, sizeof(int) * W, c->stream);
+    if (e != cudaSuccess) { set_err("ppm_chain_create: %s", cudaGetErrorString(e)); chain_free(c); return PPM_ERR_CUDA; }
+    A.lo = c->d_chain_box; A.hi = c->d_chain_box + P; A.sigma = c->d_chain_box + 2 * P; A.beta = c->d_chain_beta;
+    A.seed = seed; A.W = W; A.P = P;
+    c->chain_data = data_dev; c->chain_bkg = bkg_dev; c->chain_exposure = exposure_s;
+    if ((rc = loglike_resident(c, A.cur, W, A.ll))) { chain_free(c); return rc; }     // ln L of the starting states (also warms
+    CK(cudaStreamSynchronize(c->stream));                                               // every lazy allocation before a capture)
+    return PPM_OK;
+}
+
+static int chain_enqueue_step(ppm_ctx* c)
+{
+    const ChainArgs& A = c->chain;
+    const int blocks = (A.W + 127) / 128;
+    k_chain_propose<<<blocks, 128, 0, c->stream>>>(A);
+    int rc = loglike_resident(c, A.prop, A.W, A.llp);
+    if (rc) return rc;
+    k_chain_accept<<<blocks, 128, 0, c->stream>>>(A);
+    k_chain_swap<<<1, 256, 0, c->stream>>>(A);
+    c->launches += 3;
+    return PPM_OK;
+}
+
+extern "C" int ppm_chain_run(ppm_ctx* c, int n_steps)
+{
+    ARG(c, "null context");
+    ARG(n_steps >= 0, "n_steps must be >= 0");
+    if (!c->chain.cur) { set_err("no chain: call ppm_chain_create first"); return PPM_ERR_STATE; }
+    CK(cudaSetDevice(c->cfg.device));
+    if (n_steps == 0) return PPM_OK;
+    if (!c->stream && !c->chain_stream) {                            // the legacy default stream cannot be captured
+        CK(cudaStreamCreateWithFlags(&c->chain_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&c->chain_ev, cudaEventDisableTiming));
+    }
+    cudaStream_t user = c->stream, run = c->stream ? c->stream : c->chain_stream;
+    if (!c->chain_graph) {
+        const bool prof = c->prof_on;
+        c->prof_on = false;                                          // no event records inside the captured step
+        const int64_t l0 = c->launches;
+        cudaGraph_t graph = nullptr;
+        CK(cudaStreamBeginCapture(run, cudaStreamCaptureModeThreadLocal));
+        c->stream = run;
+        const int rc = chain_enqueue_step(c);
+        c->stream = user;
+        cudaError_t e = cudaStreamEndCapture(run, &graph);
+        c->prof_on = prof;
+        c->chain_launches_per_step = c->launches - l0;
+        c->launches = l0;
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) { set_err("capture of the sampler step failed: %s", cudaGetErrorString(e)); return PPM_ERR_CUDA; }
+        e = cudaGraphInstantiate(&c->chain_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { c->chain_graph = nullptr; set_err("cudaGraphInstantiate: %s", cudaGetErrorString(e)); return PPM_ERR_CUDA; }
+    }
+    if (run != user) {                                               // after whatever the context's stream holds ...
+        CK(cudaEventRecord(c->chain_ev, user));
+        CK(cudaStreamWaitEvent(run, c->chain_ev, 0));
+    }
+    for (int i = 0; i < n_steps; ++i) CK(cudaGraphLaunch(c->chain_graph, run));
+    if (run != user) {                                               // ... and before whatever it receives next
+        CK(cudaEventRecord(c->chain_ev, run));
+        CK(cudaStreamWaitEvent(user, c->chain_ev, 0));
+    }
+    c->launches += (int64_t)n_steps * c->chain_launches_per_step;
+    return PPM_OK;
+}
+
+extern "C" int ppm_chain_read(ppm_ctx* c, double* params, double* loglike, int64_t* accepted, int64_t* swapped, int64_t* steps)
+{
+    ARG(c, "null context");
+    if (!c->chain.cur) { set_err("no chain: call ppm_chain_create first"); return PPM_ERR_STATE; }
+    CK(cudaSetDevice(c->cfg.device));
+    if (c->chain_stream) CK(cudaStreamSynchronize(c->chain_stream));
+    CK(cudaStreamSynchronize(c->stream));
+    const ChainArgs& A = c->chain;
+    if (params) CK(cudaMemcpy(params, A.cur, sizeof(double) * A.W * A.P, cudaMemcpyDeviceToHost));
+    if (loglike) CK(cudaMemcpy(loglike, A.ll, sizeof(double) * A.W, cudaMemcpyDeviceToHost));
+    if (accepted) CK(cudaMemcpy(accepted, A.accepted, sizeof(long long) * A.W, cudaMemcpyDeviceToHost));
+    if (swapped) CK(cudaMemcpy(swapped, A.swapped, sizeof(long long) * A.W, cudaMemcpyDeviceToHost));
+    if (steps) { unsigned long long t = 0; CK(cudaMemcpy(&t, A.t, sizeof(t), cudaMemcpyDeviceToHost)); *steps = (int64_t)t; }
     return PPM_OK;
 }
 
