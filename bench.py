@@ -423,6 +423,7 @@ def main():
     clk = clocks.stop(t_begin, time.time())
     launches = ctx.launch_count() - n0
     if args.chain:                              # the captured step holds no event records: per-kernel times from eager steps
+        ctx.profile_enable(True)                # (also resets the device-side unit counter the graph replays advanced)
         timed(step, args.steps)
     prof, triples = ctx.profile_read()
     ctx.profile_enable(False)

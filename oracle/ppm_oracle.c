@@ -483,6 +483,30 @@ int orc_spot_mask(const orc_spot* sp, int n_theta, int n_phi, uint8_t* mask)
     return n;
 }
 
+/* Smallest distance of any cell of the spot's box grid from a mask decision boundary, min |cos(sep) - cos(zeta)| (and the
+ * same for the omitted cap): a cell closer than a few ulp to a boundary is decided by the last bit of cos(), which
+ * differs between math libraries -- parity tests compare such cells' masks only when this margin is comfortably large. */
+double orc_spot_mask_margin(const orc_spot* sp, int n_theta, int n_phi)
+{
+    orc_box bx; orc_spot_box(sp, n_theta, n_phi, &bx);
+    double mg = INFINITY;
+    for (int j = 0; j < n_theta; ++j) {
+        double e0 = bx.theta_lo + (bx.theta_hi - bx.theta_lo) * (double)j / n_theta;
+        double e1 = bx.theta_lo + (bx.theta_hi - bx.theta_lo) * (double)(j + 1) / n_theta;
+        double th = 0.5 * (e0 + e1), ct = cos(th), st = sin(th);
+        for (int m = 0; m < n_phi; ++m) {
+            double dphi_m = cell_dphi(&bx, m);
+            double cd = ct * cos(sp->theta_c) + st * sin(sp->theta_c) * cos(dphi_m);
+            if (fabs(cd - cos(sp->zeta)) < mg) mg = fabs(cd - cos(sp->zeta));
+            if (sp->zeta_m > 0.0) {
+                double cm = ct * cos(sp->theta_m) + st * sin(sp->theta_m) * cos(sp->phi_c + dphi_m - sp->phi_m);
+                if (fabs(cm - cos(sp->zeta_m)) < mg) mg = fabs(cm - cos(sp->zeta_m));
+            }
+        }
+    }
+    return mg;
+}
+
 /* HEALPix mask[4 nside - 1][4 nside] (1 = active; entries beyond a ring's pixel count are 0) */
 int orc_spot_mask_healpix(const orc_spot* sp, int nside, uint8_t* mask)
 {

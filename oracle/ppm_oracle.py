@@ -69,6 +69,7 @@ _star_init = _sig("orc_star_init", None, [C.c_double, C.c_double, C.c_double, C.
 _spot_box = _sig("orc_spot_box", None, [C.POINTER(Spot), C.c_int, C.c_int, C.POINTER(Box)])
 _row_init = _sig("orc_row_init", None, [C.POINTER(Star), C.POINTER(Box), C.c_int, C.c_int, C.POINTER(Row)])
 _spot_mask = _sig("orc_spot_mask", C.c_int, [C.POINTER(Spot), C.c_int, C.c_int, _u8p])
+_spot_mask_margin = _sig("orc_spot_mask_margin", C.c_double, [C.POINTER(Spot), C.c_int, C.c_int])
 _template = _sig("orc_template", C.c_int,
                  [C.POINTER(Star), C.POINTER(Row), C.c_double, C.c_double, C.c_double, C.c_int,
                   _dp, _dp, _dp, _dp, _u8p, _dp, _dp, _dp])
@@ -196,6 +197,11 @@ def spot_mask(sp, n_theta, n_phi):
     m = np.zeros((n_theta, n_phi), dtype=np.uint8)
     _spot_mask(C.byref(sp), n_theta, n_phi, m.ctypes.data_as(_u8p))
     return m
+
+
+def spot_mask_margin(sp, n_theta, n_phi):
+    """min over the box grid's cells of the distance to a mask decision boundary (in cos of the separation)."""
+    return _spot_mask_margin(C.byref(sp), n_theta, n_phi)
 
 
 def healpix_ring(nside, i):

@@ -111,7 +111,6 @@ struct ppm_ctx {
     double* d_en = nullptr;
     long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
     int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
-    int chunk = 1;                                // consecutive energies per lane chunk of k_cells_tab (1 = strided ownership)
     std::vector<double> h_en;
     // atmosphere
     bool have_atm = false;
@@ -428,25 +427,6 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
             return PPM_ERR_ARG;
         }
     }
-    // Chunked energy ownership of k_cells_tab (ppm_cells.cuh): CH consecutive energies per lane chunk share two coefficient
-    // records when every chunk spans less than one logx interval.  Instantiated for the dense-grid shapes (EPL 10 / 8, NPL 3).
-    c->chunk = 1;
-    if (c->cfg.precision == 0 && c->cfg.interp_domain == 0 && c->npl == 3 && (c->epl == 10 || c->epl == 8)) {
-        const int nE = c->cfg.n_energy, epl = c->epl;
-        for (int ch : {4, 3}) {
-            bool ok = true;
-            for (int t = 0; t < c->n_etile && ok; ++t)
-                for (int cc = 0; cc * ch < epl && ok; ++cc) {
-                    const int ncc = std::min(ch, epl - ch * cc);
-                    for (int lane = 0; lane < 32 && ok; ++lane) {
-                        const int ea = t * 32 * epl + 32 * ch * cc + ncc * lane, eb = ea + ncc - 1;
-                        if (ea >= nE) continue;
-                        ok = uef[std::min(eb, nE - 1)] - uef[ea] < (1ll << 52) - 4;
-                    }
-                }
-            if (ok) { c->chunk = ch; break; }
-        }
-    }
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
     return PPM_OK;
@@ -528,10 +508,6 @@ static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int thre
 {
     if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
     if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
-    if constexpr (EPL == 10 || EPL == 8) {
-        if (c->npl == 3 && c->chunk == 4) return launch_cells(c, k_cells_tab<EPL, 3, 4>, a, grid, threads, smem);
-        if (c->npl == 3 && c->chunk == 3) return launch_cells(c, k_cells_tab<EPL, 3, 3>, a, grid, threads, smem);
-    }
     switch (c->npl) {
     case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
     case 3:  return launch_cells(c, k_cells_tab<EPL, 3>, a, grid, threads, smem);

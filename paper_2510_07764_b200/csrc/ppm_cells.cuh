@@ -442,61 +442,7 @@ __device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], c
     else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1>(g, acc, uef, KAq, q, s_top);
 }
 
-// ---- chunked energy ownership (CH > 1) -----------------------------------------------------------
-// A lane's EPL energies are split into chunks of CH CONSECUTIVE energies (the last chunk takes the remainder):
-//   energy index of (chunk c, lane, r) = e0 + 32 CH c + n_c lane + r,   n_c = min(CH, EPL - CH c),   i = CH c + r.
-// The host selects CH > 1 only when every chunk spans less than one logx interval (ppm_load_atmosphere), so all energies
-// of a chunk lie in the interval j of its first energy or in j + 1: the two coefficient records are loaded ONCE per chunk
-// (4 LDS.128) and each energy picks one of them in registers -- 16 n_chunks / EPL shared-memory wavefronts per triple
-// instead of 8 (the kernel is bound by shared-memory bandwidth: profiles/r2_k_cells_tab.md).
-template <int EPL, int CH>
-__device__ __forceinline__ int chunk_energy(int e0, int lane, int i)
-{
-    const int c = i / CH, r = i - c * CH;
-    const int nc = (EPL - CH * c < CH) ? EPL - CH * c : CH;
-    return e0 + 32 * CH * c + nc * lane + r;
-}
-
-// chunks 0 .. G-1 of a pair; CLAMP: the last of them may straddle the top of the axis and clamps its coordinates
-template <int KW, int EPL, int CH, int G, bool CLAMP>
-__device__ __forceinline__ void energies_chunked(double (&acc)[EPL], const long long (&uef)[EPL],
-                                                 const double2* __restrict__ KAq, long long q, long long s_top)
-{
-#pragma unroll
-    for (int c = 0; c < G; ++c) {
-        const int i0 = CH * c;
-        const int nc = (EPL - i0 < CH) ? EPL - i0 : CH;
-        long long s0 = q + uef[i0];                                         // first energy of the lane's chunk
-        if (CLAMP && c == G - 1) s0 = s0 > s_top ? s_top : s0;              // (only lane 0's is known to be inside the table)
-        const int j = (int)(s0 >> 52);
-        const double2* kp = KAq + j;
-        const double2 a01 = kp[0], a23 = kp[KW], b01 = kp[1], b23 = kp[KW + 1];
-#pragma unroll
-        for (int r = 0; r < CH; ++r) {
-            if (r >= nc) break;
-            long long s = q + uef[i0 + r];
-            if (CLAMP && c == G - 1) s = s > s_top ? s_top : s;
-            const int shi = (int)(s >> 32);
-            const bool up = (r > 0) && ((shi >> 20) != j);                  // interval j + 1
-            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
-            const double k0 = up ? b01.x : a01.x, k1 = up ? b01.y : a01.y;
-            const double k2 = up ? b23.x : a23.x, k3 = up ? b23.y : a23.y;
-            const double y = fma(fma(fma(k3, tau, k2), tau, k1), tau, k0);
-            const double rr = y + kMagic;
-            acc[i0 + r] += exp2_frac_scaled(y - (rr - kMagic), __double2loint(rr));
-        }
-    }
-}
-
-template <int KW, int EPL, int CH, int G>
-__device__ __forceinline__ void dispatch_chunked_hi(int g, double (&acc)[EPL], const long long (&uef)[EPL],
-                                                    const double2* __restrict__ KAq, long long q, long long s_top)
-{
-    if (g == G) energies_chunked<KW, EPL, CH, G, true>(acc, uef, KAq, q, s_top);
-    else if constexpr (G > 1) dispatch_chunked_hi<KW, EPL, CH, G - 1>(g, acc, uef, KAq, q, s_top);
-}
-
-template <int EPL, int NPL, int CH = 1>
+template <int EPL, int NPL>
 __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
@@ -524,15 +470,14 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
     double* T = S + plane;
     double* MUAX = T + 4 * n1;
     long long* UG = reinterpret_cast<long long*>(MUAX + A.nmu);                 // [NG]: coordinate part of each group's first energy
-    // energy groups: CH == 1: group i = the 32 energies e0 + lane + 32 i (strided ownership); CH > 1: group c = chunk c, the
-    // 32 n_c consecutive energies from e0 + 32 CH c (chunked ownership).  Either way energies rise with the group index.
-    constexpr int NG = (CH == 1) ? EPL : (EPL + CH - 1) / CH;
+    // energy group i = the 32 consecutive energies e0 + 32 i + lane: energies rise with the group index and with the lane
+    constexpr int NG = EPL;
 
     long long uef[EPL];
     double acc[EPL];
 #pragma unroll
     for (int i = 0; i < EPL; ++i) {
-        const int e = (CH == 1) ? e0 + lane + 32 * i : chunk_energy<EPL, CH>(e0, lane, i);
+        const int e = e0 + lane + 32 * i;
         uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
         acc[i] = 0.0;
     }
@@ -542,7 +487,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
     const long long s_top = ((long long)(nx - 1) << 52) - 1;                     // largest in-table coordinate
     for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
     if (threadIdx.x < NG) {                      // a group without any energy (ragged tail) counts as beyond the table
-        const int ef = e0 + 32 * (CH == 1 ? 1 : CH) * (int)threadIdx.x;
+        const int ef = e0 + 32 * (int)threadIdx.x;
         UG[threadIdx.x] = (ef < A.nE) ? A.uef[ef] : (1ll << 62);
     }
 
@@ -631,14 +576,9 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                     // every coordinate of the tile lies inside the table and every exponent is in range
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
-                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52), sizeof(double2) * (CH == 1 ? 1 : 2));
-                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52) + KW, sizeof(double2) * (CH == 1 ? 1 : 2));
-                    }
-                    if constexpr (CH == 1) {
-#pragma unroll
-                        for (int i = 0; i < EPL; ++i) acc[i] += triple_value<KW>(KAq, q + uef[i]);
-                    } else {
-                        energies_chunked<KW, EPL, CH, NG, false>(acc, uef, KAq, q, s_top);
+                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52), sizeof(double2));
+                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52) + KW, sizeof(double2));
+                        acc[i] += triple_value<KW>(KAq, q + uef[i]);
                     }
                 } else if ((flg & 7) == PAIR_CLAMP_HI) {
                     // the upper energies lie beyond the top of the logx axis: the clamped coordinate (reading R13b) makes
@@ -649,8 +589,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         const double vtop = triple_value<KW>(KAq, s_top);
                         if (lane == g) hdef += vtop;
                     }
-                    if constexpr (CH == 1) dispatch_clamped_hi<KW, EPL, EPL>(g, acc, uef, KAq, q, s_top);
-                    else dispatch_chunked_hi<KW, EPL, CH, NG>(g, acc, uef, KAq, q, s_top);
+                    dispatch_clamped_hi<KW, EPL, EPL>(g, acc, uef, KAq, q, s_top);
                 } else {
                     // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
                     // range-checked form
@@ -668,12 +607,12 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
         if (lane >= d) hdef += up;
     }
 #pragma unroll
-    for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, CH == 1 ? i : i / CH);
+    for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, i);
     if (kvalid) {
         double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
-            const int e = (CH == 1) ? e0 + lane + 32 * i : chunk_energy<EPL, CH>(e0, lane, i);
+            const int e = e0 + lane + 32 * i;
             if (e < A.nE) out[e] = acc[i] / A.en[e];                            // the 1/E_e of Eq 47
         }
     }
