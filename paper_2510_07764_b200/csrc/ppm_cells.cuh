@@ -71,23 +71,18 @@ __global__ void __launch_bounds__(256) k_slice(SliceArgs A)
 // 2^f by a degree-8 polynomial (Chebyshev-node fit on [-1/2, 1/2]; max relative error 1.1e-12 -- three orders
 // below the 1e-9 per-bin parity bar; degree 10 reaches 4e-16 at +2 DFMA per triple, measured 6 % slower),
 // 2^n by an integer add into the exponent field.  The caller drops terms with n < -1000.
-// The coefficients sit in the constant bank: every DFMA of the Horner chain takes its addend straight from c[][]
-// (no register, no per-pair re-materialisation of 18 words).
-__constant__ double c_exp2[9] = {1.3255224878668817e-06, 1.5310079402249296e-05, 0.00015403455852453838,
-                                 0.0013333450568000645,  0.009618129159402558,   0.05550410941205933,
-                                 0.2402265069581299,     0.6931471805459335,     1.0};
-
+// (Literal coefficients: measured faster than operands from the constant bank -- C5 x 8 54.3 vs 56.3 ms, maps 11.5 vs 13.0 ms.)
 __device__ __forceinline__ double exp2_frac_scaled(double f, int n)      // 2^f * 2^n, |f| <= 1/2, no range check
 {
-    double p = c_exp2[0];
-    p = fma(p, f, c_exp2[1]);
-    p = fma(p, f, c_exp2[2]);
-    p = fma(p, f, c_exp2[3]);
-    p = fma(p, f, c_exp2[4]);
-    p = fma(p, f, c_exp2[5]);
-    p = fma(p, f, c_exp2[6]);
-    p = fma(p, f, c_exp2[7]);
-    p = fma(p, f, c_exp2[8]);
+    double p = 1.3255224878668817e-06;
+    p = fma(p, f, 1.5310079402249296e-05);
+    p = fma(p, f, 0.00015403455852453838);
+    p = fma(p, f, 0.0013333450568000645);
+    p = fma(p, f, 0.009618129159402558);
+    p = fma(p, f, 0.05550410941205933);
+    p = fma(p, f, 0.2402265069581299);
+    p = fma(p, f, 0.6931471805459335);
+    p = fma(p, f, 1.0);
     return __hiloint2double(__double2hiint(p) + n * 1048576, __double2loint(p));
 }
 

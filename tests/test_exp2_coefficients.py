@@ -1,4 +1,4 @@
-"""CPU check of the degree-8 polynomial the table cell kernel uses for 2^f, |f| <= 1/2 (ppm_cells.cuh: c_exp2): the
+"""CPU check of the degree-8 polynomial the table cell kernel uses for 2^f, |f| <= 1/2 (ppm_cells.cuh: exp2_frac_scaled): the
 coefficients are parsed from the CUDA source and evaluated in the kernel's Horner order against numpy.exp2; the claimed
 bound (max relative error 1.1e-12, three orders below the 1e-9 parity bar) is asserted.  Also the FP32 helper constants."""
 import os
@@ -11,8 +11,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def _coefficients():
     src = open(os.path.join(ROOT, "paper_2510_07764_b200", "csrc", "ppm_cells.cuh")).read()
-    body = re.search(r"__constant__ double c_exp2\[9\]\s*=\s*\{(.*?)\};", src, flags=re.S).group(1)
-    c = [float(x) for x in re.findall(r"[-+]?\d+\.\d+(?:[eE][-+]?\d+)?|[-+]?\d+\.(?![\d])", body)]
+    body = re.search(r"double exp2_frac_scaled\(double f, int n\).*?\{(.*?)return", src, flags=re.S).group(1)
+    c = [float(x) for x in re.findall(r"(?:double p = |fma\(p, f, )([-+]?\d+\.?\d*(?:[eE][-+]?\d+)?)", body)]
     assert len(c) == 9
     return c
 
