@@ -297,16 +297,22 @@ __device__ __forceinline__ double node_value(const double* __restrict__ sp0, int
     return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], fma(v0, sp0[0], qb))));
 }
 
-// monomial coefficients (in tau, the offset from the interval midpoint in units of h) of the cubic through
-// the node values c0..c3 at tau = -3/2, -1/2, 1/2, 3/2
-__device__ __forceinline__ void cubic_coeffs(double c0, double c1, double c2, double c3, double& k0, double& k1,
-                                             double& k2, double& k3)
+// monomial coefficients, in t = 1 + (fraction of the interval) -- t runs over [1, 2) across the interval between the
+// nodes c1 and c2; the four nodes sit at t = 0, 1, 2, 3 -- of the cubic through the node values c0..c3: Newton's forward
+// differences (differences of neighbouring nodes first: no cancellation against the nodes' common magnitude) turned
+// into monomials.  t is what the fixed-point coordinate yields directly (fraction bits under the exponent of 1.0), so a
+// triple needs no subtraction to centre it.  Neighbouring intervals of a lane share their first and second differences.
+__device__ __forceinline__ void cubic_coeffs(double c0, double c1, double c2, double c3, double& a0, double& a1,
+                                             double& a2, double& a3)
 {
-    const double s03 = c0 + c3, s12 = c1 + c2, d30 = c3 - c0, d21 = c2 - c1;
-    k0 = fma(s03, -0.0625, s12 * 0.5625);
-    k1 = fma(d30, -1.0 / 24.0, d21 * 1.125);
-    k2 = (s03 - s12) * 0.25;
-    k3 = fma(d21, -0.5, d30 * (1.0 / 6.0));
+    const double d1 = c1 - c0, d2 = c2 - c1, d3 = c3 - c2;
+    const double e1 = d2 - d1, e2 = d3 - d2;
+    const double t3 = e2 - e1;
+    const double h2 = 0.5 * e1;
+    a0 = c0;
+    a1 = d1 - fma(t3, -1.0 / 3.0, h2);
+    a2 = fma(t3, -0.5, h2);
+    a3 = t3 * (1.0 / 6.0);
 }
 
 // debug build (-DPPM_BOUNDS): every shared-memory access of the table cell kernel is checked against the block's
@@ -360,7 +366,8 @@ __device__ __forceinline__ void fused_pass(const double* __restrict__ srow, int 
             const int c = n0 + jn;
             if (c != 0 && c != nx - 2) continue;
             if (x_linedge) {                                        // strategies c, d: linear
-                ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
+                const double d = f[jn + 2] - f[jn + 1];             // y = f1 + d (t - 1)
+                ka[jn] = make_double2(f[jn + 1] - d, d);
                 kb[jn] = make_double2(0.0, 0.0);
             } else {                                                // strategies a, b: stencil shifted inward
                 const int s = (c == 0) ? 0 : nx - 4;
@@ -369,7 +376,7 @@ __device__ __forceinline__ void fused_pass(const double* __restrict__ srow, int 
                 for (int m = 0; m < 4; ++m) g[m] = node_value(srow + s + m, nx, v0, v1, v2, v3, qb);
                 double k0, k1, k2, k3;
                 cubic_coeffs(g[0], g[1], g[2], g[3], k0, k1, k2, k3);
-                const double d = (double)(c - 1 - s);               // Taylor shift to this interval's midpoint
+                const double d = (double)(c - 1 - s);               // Taylor shift: this interval is [1, 2) of its own t
                 ka[jn] = make_double2(fma(d, fma(d, fma(d, k3, k2), k1), k0), fma(d, fma(3.0 * d, k3, 2.0 * k2), k1));
                 kb[jn] = make_double2(fma(3.0 * d, k3, k2), k3);
             }
@@ -390,9 +397,9 @@ __device__ __forceinline__ double triple_value(const double2* __restrict__ KAq, 
 {
     const int shi = (int)(s >> 32);
     const double2* kp = KAq + (shi >> 20);                                      // interval index = s >> 52
-    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+    const double t = __hiloint2double(one_plus_frac_hi(shi), (int)s);              // 1 + fraction of the interval
     const double2 c01 = kp[0], c23 = kp[KW];
-    const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+    const double y = fma(fma(fma(c23.y, t, c23.x), t, c01.y), t, c01.x);
     const double r = y + kMagic;
     return exp2_frac_scaled(y - (r - kMagic), __double2loint(r));
 }
@@ -405,9 +412,9 @@ __device__ __forceinline__ double triple_value_checked(const double2* __restrict
     s = s < 0 ? 0 : (s > s_top ? s_top : s);
     const int shi = (int)(s >> 32);
     const double2* kp = KAq + (shi >> 20);
-    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+    const double t = __hiloint2double(one_plus_frac_hi(shi), (int)s);              // 1 + fraction of the interval
     const double2 c01 = kp[0], c23 = kp[KW];
-    const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
+    const double y = fma(fma(fma(c23.y, t, c23.x), t, c01.y), t, c01.x);
     const double r = y + kMagic;
     const int n = __double2loint(r);
     const double v = exp2_frac_scaled(y - (r - kMagic), n);

@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_lin(CellArgs A)
                     s = s < 0 ? 0 : (s > s_top ? s_top : s);                     // clamp to the table (reading R13b)
                     const int shi = (int)(s >> 32);
                     const double2* kp = KAq + (shi >> 20);
-                    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                    const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s);   // t = 1 + fraction (see cubic_coeffs)
                     const double2 c01 = kp[0], c23 = kp[KW];
                     double v = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);   // F_p T^3 * (I/T^3)
                     if (clip) v = fmax(v, 0.0);                                  // strategy b

@@ -234,7 +234,8 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                         for (int jn = 0; jn < NPL; ++jn) {
                             const int c = n0 + jn;
                             if (c != 0 && c != nx - 2) continue;
-                            ka[jn] = make_double2(0.5 * (f[jn + 1] + f[jn + 2]), f[jn + 2] - f[jn + 1]);
+                            const double d = f[jn + 2] - f[jn + 1];             // y = f1 + d (t - 1)
+                            ka[jn] = make_double2(f[jn + 1] - d, d);
                             kb[jn] = make_double2(0.0, 0.0);
                         }
                     }
@@ -252,7 +253,7 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                             const long long s = q + uef[i];
                             const int shi = (int)(s >> 32);
                             const double2* kp = KAq + (shi >> 20);
-                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s);   // t = 1 + fraction (see cubic_coeffs)
                             const double2 c01 = kp[0], c23 = kp[KW];
                             const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
                             const double r = y + kMagic;
@@ -267,7 +268,7 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                             s = s < 0 ? 0 : (s > s_top ? s_top : s);             // clamp to the table (reading R13b)
                             const int shi = (int)(s >> 32);
                             const double2* kp = KAq + (shi >> 20);
-                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s) - 1.5;
+                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s);   // t = 1 + fraction (see cubic_coeffs)
                             const double2 c01 = kp[0], c23 = kp[KW];
                             const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
                             const double r = y + kMagic;
