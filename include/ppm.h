@@ -188,6 +188,10 @@ int64_t ppm_launch_count(const ppm_ctx* ctx);
 /* Vectors per internal sub-batch (scratch_mb / per-vector scratch, capped by max_batch); a batch B is processed
  * as ceil(B / ppm_sub_batch) sequences of launches.  Final after ppm_load_atmosphere for table emission. */
 int ppm_sub_batch(const ppm_ctx* ctx);
+/* 1 if the context's energy grid is log-uniform to within 256 units of 2^-52 table intervals, so that the table cell
+ * kernel steps its logx coordinate from energy group to energy group instead of holding one value per energy
+ * ("uniform energy path"); 0 otherwise or before ppm_load_atmosphere. */
+int ppm_uniform_energy(const ppm_ctx* ctx);
 /* Effective n_fp after defaulting. */
 int ppm_n_fp(const ppm_ctx* ctx);
 

@@ -49,6 +49,7 @@ EXPORTS = {
     "ppm_launch_count": (C.c_int64, [_vp]),
     "ppm_n_fp": (C.c_int, [_vp]),
     "ppm_sub_batch": (C.c_int, [_vp]),
+    "ppm_uniform_energy": (C.c_int, [_vp]),
     "ppm_profile_enable": (C.c_int, [_vp, C.c_int]),
     "ppm_profile_read": (C.c_int, [_vp, _dp, C.POINTER(C.c_int64), _dp]),
     "ppm_measure_fp64_peak": (C.c_int, [C.c_int, _dp]),
@@ -345,3 +346,6 @@ class PPM:
 
     def sub_batch(self):
         return int(self.lib.ppm_sub_batch(self._h))
+
+    def uniform_energy(self):
+        return bool(self.lib.ppm_uniform_energy(self._h))

@@ -111,6 +111,8 @@ struct ppm_ctx {
     double* d_en = nullptr;
     long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
     int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
+    bool uniform_e = false;                       // log-uniform energy grid: the cell kernels step the coordinate (EnergyCoord)
+    long long uef_step = 0;                       // 32 * the grid's step of uef
     std::vector<double> h_en;
     // atmosphere
     bool have_atm = false;
@@ -331,6 +333,7 @@ extern "C" int ppm_create(const ppm_config* cfg, const double* energies, void* s
 
 extern "C" int ppm_n_fp(const ppm_ctx* c) { return c ? c->n_fp : 0; }
 extern "C" int ppm_sub_batch(const ppm_ctx* c) { return c ? c->SB : 0; }
+extern "C" int ppm_uniform_energy(const ppm_ctx* c) { return (c && c->uniform_e) ? 1 : 0; }
 extern "C" int64_t ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }
 
 extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const double* logg, int ng,
@@ -426,6 +429,24 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
             set_err("table (%d x %d) + template (n_fp = %d) do not fit the cell kernel's shared memory", nmu, nx, c->n_fp);
             return PPM_ERR_ARG;
         }
+        // Log-uniform energy grid?  Then energy e0 + lane + 32 i of a tile is evaluated at uef[e0 + lane] + i * step32 (see
+        // EnergyCoord in ppm_cells.cuh).  Taken only if that affine form is within 256 units of 2^-52 table intervals of
+        // every energy's own coordinate and only the last group of every tile is ragged.
+        c->uniform_e = false; c->uef_step = 0;
+        const int nE = c->cfg.n_energy;
+        if (nE > 32 && c->epl >= 2) {
+            const long long step32 = llrintl(32.0L * (long double)(uef[nE - 1] - uef[0]) / (long double)(nE - 1));
+            bool ok = step32 > 0;
+            for (int t = 0; t < c->n_etile && ok; ++t) {
+                const int ea = t * 32 * c->epl, nt = std::min(nE, ea + 32 * c->epl) - ea;
+                if (nt <= 32 * (c->epl - 1)) ok = false;            // more than the last group would be ragged
+                for (int k = 0; k < nt && ok; ++k) {
+                    const long long dev = uef[ea + k] - (uef[ea + (k & 31)] + (long long)(k >> 5) * step32);
+                    if (dev > 256 || dev < -256) ok = false;
+                }
+            }
+            if (ok) { c->uniform_e = true; c->uef_step = step32; }
+        }
     }
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
@@ -508,12 +529,23 @@ static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int thre
 {
     if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
     if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
+    if constexpr (EPL >= 2) {
+        if (a.uniform_e) {
+            switch (c->npl) {
+            case 1:  return launch_cells(c, k_cells_tab<EPL, 1, true>, a, grid, threads, smem);
+            case 3:  return launch_cells(c, k_cells_tab<EPL, 3, true>, a, grid, threads, smem);
+            case 5:  return launch_cells(c, k_cells_tab<EPL, 5, true>, a, grid, threads, smem);
+            case 7:  return launch_cells(c, k_cells_tab<EPL, 7, true>, a, grid, threads, smem);
+            default: return launch_cells(c, k_cells_tab<EPL, 9, true>, a, grid, threads, smem);
+            }
+        }
+    }
     switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_tab<EPL, 1>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_tab<EPL, 3>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_tab<EPL, 5>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_tab<EPL, 7>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_tab<EPL, 9>, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells_tab<EPL, 1, false>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_tab<EPL, 3, false>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_tab<EPL, 5, false>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_tab<EPL, 7, false>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_tab<EPL, 9, false>, a, grid, threads, smem);
     }
 }
 
@@ -599,6 +631,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     CellArgs A{};
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
     A.slices = c->d_slices; A.axmu = c->d_axmu; A.uef = c->d_uef; A.en = c->d_en;
+    A.uniform_e = (table && c->uniform_e) ? 1 : 0; A.uef_step = c->uef_step;
     A.partial = c->d_partial; A.pairs = c->d_pairs;
     A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;

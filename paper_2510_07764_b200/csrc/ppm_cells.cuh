@@ -15,6 +15,8 @@ struct CellArgs {
     const double* axmu;      // [nmu]
     const long long* uef;    // [nE]: round(log10(E_e) / h * 2^52): energy part of the logx coordinate in fixed point
                              //       (h = logx spacing; units of 2^-52 table intervals)
+    long long uef_step;      // log-uniform energy grids (uniform_e = 1): 32 * the grid's constant step of uef (see EnergyCoord)
+    int uniform_e;
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
     const double* tmap;      // temperature-map mode: [rows][n_phi] log10 T per cell
@@ -421,30 +423,67 @@ __device__ __forceinline__ double triple_value_checked(const double2* __restrict
     return !(y > -1000.0) ? 0.0 : (y > 1000.0 ? INFINITY : v);
 }
 
+// The energy part of the logx coordinate for the EPL energies e0 + lane + 32 i a lane owns.
+//  UNI = false: one 64-bit value per energy in registers (2 EPL registers).
+//  UNI = true (log-uniform energy grid -- the paper's grids are, Eq 50): energy i sits at uef[e0 + lane] + i D with
+//  ONE warp-uniform step D = 32 * (step of uef), so a lane carries its coordinate from group to group by one 64-bit add
+//  and the 2 EPL registers become 2.  The host takes this path only when every energy's own uef differs from that
+//  affine form by <= 256 units of 2^-52 intervals (5.7e-14 of a table interval: a relative change of the energy of 2.6e-15,
+//  ~ 12 ulp of a double; worst-case effect on a term 2.6e-13, the seeded grids deviate by <= 105 units) and when only the
+//  last group of a tile is ragged; a lane whose last energy does not exist re-evaluates its previous one (Dlast = 0; the
+//  result is never stored).
+template <int EPL, bool UNI>
+struct EnergyCoord {
+    long long u[UNI ? 1 : EPL];
+    long long D, Dlast;
+    __device__ __forceinline__ void init(const long long* __restrict__ uef, long long step, int e0, int lane, int nE)
+    {
+        if constexpr (UNI) {
+            u[0] = uef[imin_(e0 + lane, nE - 1)];
+            D = step;
+            Dlast = (e0 + lane + 32 * (EPL - 1) < nE) ? step : 0;
+        } else {
+#pragma unroll
+            for (int i = 0; i < EPL; ++i) u[i] = uef[imin_(e0 + lane + 32 * i, nE - 1)];
+            D = Dlast = 0;
+        }
+    }
+    __device__ __forceinline__ long long first(long long q) const { return q + u[0]; }
+    // coordinate of group i + 1 given s = that of group i
+    __device__ __forceinline__ long long next(long long s, long long q, int i) const
+    {
+        if constexpr (UNI) return s + ((i == EPL - 2) ? Dlast : D);
+        else return q + u[i + 1 < EPL ? i + 1 : EPL - 1];
+    }
+};
+
 // Energies of a pair whose upper part lies beyond the top of the logx axis.  The lane's energies e0 + lane + 32 i rise
 // with i and with the lane, so the groups i >= G (G warp-uniform: the groups whose FIRST energy is still inside the table)
 // are clamped for every lane: their term is the pair's constant 2^y(s_top) and is not evaluated here (the caller defers it).
 // Groups i < G - 1 are entirely inside the table; group G - 1 may straddle the end and clamps its coordinate.
 // One fully unrolled instance per G keeps the G independent dependency chains interleaved.
-template <int KW, int EPL, int G>
-__device__ __forceinline__ void energies_clamped_hi(double (&acc)[EPL], const long long (&uef)[EPL],
+template <int KW, int EPL, int G, bool UNI>
+__device__ __forceinline__ void energies_clamped_hi(double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec,
                                                     const double2* __restrict__ KAq, long long q, long long s_top)
 {
+    long long s = ec.first(q);
 #pragma unroll
-    for (int i = 0; i < G - 1; ++i) acc[i] += triple_value<KW>(KAq, q + uef[i]);
-    const long long s = q + uef[G - 1];
+    for (int i = 0; i < G - 1; ++i) {
+        acc[i] += triple_value<KW>(KAq, s);
+        s = ec.next(s, q, i);
+    }
     acc[G - 1] += triple_value<KW>(KAq, s > s_top ? s_top : s);
 }
 
-template <int KW, int EPL, int G>
-__device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], const long long (&uef)[EPL],
+template <int KW, int EPL, int G, bool UNI>
+__device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec,
                                                     const double2* __restrict__ KAq, long long q, long long s_top)
 {
-    if (g == G) energies_clamped_hi<KW, EPL, G>(acc, uef, KAq, q, s_top);
-    else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1>(g, acc, uef, KAq, q, s_top);
+    if (g == G) energies_clamped_hi<KW, EPL, G, UNI>(acc, ec, KAq, q, s_top);
+    else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1, UNI>(g, acc, ec, KAq, q, s_top);
 }
 
-template <int EPL, int NPL>
+template <int EPL, int NPL, bool UNI>
 __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
@@ -475,22 +514,23 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
     // energy group i = the 32 consecutive energies e0 + 32 i + lane: energies rise with the group index and with the lane
     constexpr int NG = EPL;
 
-    long long uef[EPL];
+    EnergyCoord<EPL, UNI> ec;
+    ec.init(A.uef, A.uef_step, e0, lane, A.nE);
     double acc[EPL];
 #pragma unroll
-    for (int i = 0; i < EPL; ++i) {
-        const int e = e0 + lane + 32 * i;
-        uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
-        acc[i] = 0.0;
-    }
+    for (int i = 0; i < EPL; ++i) acc[i] = 0.0;
     double hdef = 0.0;                           // lane g: sum of the constants 2^y(s_top) of the pairs whose groups >= g are clamped
+    // first / last coordinate of the tile's energies, in the same form the lanes use (EnergyCoord): the coordinates are
+    // monotone in the energy index, so every index the energy loop forms lies inside the window found from these two
     const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
-    const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
+    const int e_last = imin_(e0 + 32 * EPL, A.nE) - 1;
+    const long long uef_last = UNI ? A.uef[e0 + ((e_last - e0) & 31)] + (long long)((e_last - e0) >> 5) * A.uef_step
+                                   : A.uef[e_last];
     const long long s_top = ((long long)(nx - 1) << 52) - 1;                     // largest in-table coordinate
     for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
     if (threadIdx.x < NG) {                      // a group without any energy (ragged tail) counts as beyond the table
         const int ef = e0 + 32 * (int)threadIdx.x;
-        UG[threadIdx.x] = (ef < A.nE) ? A.uef[ef] : (1ll << 62);
+        UG[threadIdx.x] = (ef < A.nE) ? (UNI ? A.uef[e0] + (long long)threadIdx.x * A.uef_step : A.uef[ef]) : (1ll << 62);
     }
 
     const StarD& st = A.stars[b];
@@ -576,11 +616,13 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 // ---- energies ----
                 if (flg == 0) {
                     // every coordinate of the tile lies inside the table and every exponent is in range
+                    long long s = ec.first(q);
 #pragma unroll
                     for (int i = 0; i < EPL; ++i) {
-                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52), sizeof(double2));
-                        PPM_SMEM_CHECK(KAq + ((q + uef[i]) >> 52) + KW, sizeof(double2));
-                        acc[i] += triple_value<KW>(KAq, q + uef[i]);
+                        PPM_SMEM_CHECK(KAq + (s >> 52), sizeof(double2));
+                        PPM_SMEM_CHECK(KAq + (s >> 52) + KW, sizeof(double2));
+                        acc[i] += triple_value<KW>(KAq, s);
+                        s = ec.next(s, q, i);
                     }
                 } else if ((flg & 7) == PAIR_CLAMP_HI) {
                     // the upper energies lie beyond the top of the logx axis: the clamped coordinate (reading R13b) makes
@@ -591,12 +633,16 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                         const double vtop = triple_value<KW>(KAq, s_top);
                         if (lane == g) hdef += vtop;
                     }
-                    dispatch_clamped_hi<KW, EPL, EPL>(g, acc, uef, KAq, q, s_top);
+                    dispatch_clamped_hi<KW, EPL, EPL, UNI>(g, acc, ec, KAq, q, s_top);
                 } else {
                     // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
                     // range-checked form
+                    long long s = ec.first(q);
 #pragma unroll
-                    for (int i = 0; i < EPL; ++i) acc[i] += triple_value_checked<KW>(KAq, q + uef[i], s_top);
+                    for (int i = 0; i < EPL; ++i) {
+                        acc[i] += triple_value_checked<KW>(KAq, s, s_top);
+                        s = ec.next(s, q, i);
+                    }
                 }
             }
         }

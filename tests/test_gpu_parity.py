@@ -247,6 +247,44 @@ def test_table_edges_below_and_above_the_logx_axis(emission):
     assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
 
 
+@pytest.mark.parametrize("emission", [1, 2])
+def test_table_edges_on_the_uniform_energy_path(emission):
+    """The same sweep across both ends of the logx axis with 320 energies = one full tile of a log-uniform grid: the cell
+    kernel steps its coordinate from energy group to energy group (EnergyCoord, UNI = true) through the clamped-low,
+    the plain and the clamped-high energy loops."""
+    conf = gen.config_c2(n_cells=20, n_phase=19, n_energy=320)
+    conf["cfg"] = dict(conf["cfg"], emission=emission)
+    conf["energies"] = gen.logspace(0.002, 40.0, 320)
+    conf["params"] = conf["params"].copy()
+    conf["params"][0, 8 + 3] = 6.45
+    g, st, ctx = gpu_flux(conf)
+    assert ctx.uniform_energy()
+    ref, _ = oracle_flux(conf)
+    assert st[0] == 0 and max_rel_err(g[0], ref) <= TOL
+
+
+def test_uniform_and_general_energy_paths():
+    """Log-uniform grids (all BASELINE.json configs) take the stepped-coordinate kernel, with a ragged last energy group
+    (120 = 3 x 32 + 24 energies); a grid that is uniform in E (an instrument's channel grid) is not log-uniform and takes
+    the kernel that holds one coordinate per energy.  Both against the oracle."""
+    for name in ("c2", "c3", "c4"):
+        small = getattr(gen, "config_" + name)(n_cells=8, n_phase=8)
+        assert make_ctx(small).uniform_energy(), name
+    assert make_ctx(gen.config_t()).uniform_energy()
+    conf = gen.config_c3(n_cells=24, n_phase=20, n_energy=120)
+    g, st, ctx = gpu_flux(conf)
+    assert ctx.uniform_energy()
+    ref, _ = oracle_flux(conf)
+    e_uni = max_rel_err(g[0], ref)
+    lin = dict(conf, energies=np.linspace(0.25, 9.0, 120))
+    g2, st2, ctx2 = gpu_flux(lin)
+    assert not ctx2.uniform_energy()
+    ref2, _ = oracle_flux(lin)
+    e_gen = max_rel_err(g2[0], ref2)
+    report("energy_paths", uniform=e_uni, general=e_gen)
+    assert st[0] == 0 and st2[0] == 0 and e_uni <= TOL and e_gen <= TOL
+
+
 def test_narrow_energy_band_uses_a_small_window():
     """8 energies in a narrow band: the per-pair window is a few intervals (NPL = 1 variant of the cell kernel)."""
     conf = gen.config_c3(n_cells=24, n_phase=16, n_energy=8)
