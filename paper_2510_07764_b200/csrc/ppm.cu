@@ -138,7 +138,8 @@ struct ppm_ctx {
     std::vector<cudaEvent_t> prof_ev;             // pool, two per recorded launch
     std::vector<int> prof_kid;                    // kernel id of each recorded launch
     size_t prof_used = 0;
-    unsigned long long* d_pairs = nullptr;        // (cell, phase) pairs with F_p != 0 walked by k_cells
+    unsigned long long* d_pairs = nullptr;        // [0] (cell, phase) pairs with F_p != 0 walked by k_cells; [1] temperature-map
+                                                  // mode: rows left to the full-width launch
     // device-resident sampler loop (ppm_chain_*)
     ChainArgs chain{};
     double* d_chain_box = nullptr;                // lo | hi | sigma [3][P]
@@ -248,8 +249,8 @@ static int alloc_scratch(ppm_ctx* c)
     if ((rc = dev_alloc(&c->d_lookup, rows * 2 * kNCheb))) return rc;
     if ((rc = dev_alloc(&c->d_tmpl, rows * 4 * (c->n_fp + 1)))) return rc;
     if ((rc = dev_alloc(&c->d_partial, (size_t)c->SB * c->nchunk * g.n_phase * g.n_energy))) return rc;
-    if ((rc = dev_alloc(&c->d_pairs, (size_t)1))) return rc;
-    if (cudaMemsetAsync(c->d_pairs, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return PPM_ERR_CUDA;
+    if ((rc = dev_alloc(&c->d_pairs, (size_t)2))) return rc;
+    if (cudaMemsetAsync(c->d_pairs, 0, 2 * sizeof(unsigned long long), c->stream) != cudaSuccess) return PPM_ERR_CUDA;
     return PPM_OK;
 }
 
@@ -574,19 +575,30 @@ static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, 
 // shared memory of k_cells_map with `nw` warps (ppm_cells_map.cuh layout)
 static size_t cells_map_smem(const ppm_ctx* c, int nw, int wst)
 {
-    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 16) + 2 * (size_t)c->nmu * wst +
-                             4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT);
+    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 32) + 2 * (size_t)c->nmu * wst +
+                             4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT + 16);
 }
 
 template <int EPL, bool WIN>
 static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
+    if constexpr (WIN && EPL >= 4) {                                    // the stepped coordinate (EnergyCoord): windowed kernel only
+        if (a.uniform_e) {
+            switch (c->npl) {
+            case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN, true>, a, grid, threads, smem);
+            case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN, true>, a, grid, threads, smem);
+            case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN, true>, a, grid, threads, smem);
+            case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN, true>, a, grid, threads, smem);
+            default: return launch_cells(c, k_cells_map<EPL, 9, WIN, true>, a, grid, threads, smem);
+            }
+        }
+    }
     switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_map<EPL, 9, WIN>, a, grid, threads, smem);
+    case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN, false>, a, grid, threads, smem);
+    case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN, false>, a, grid, threads, smem);
+    case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN, false>, a, grid, threads, smem);
+    case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN, false>, a, grid, threads, smem);
+    default: return launch_cells(c, k_cells_map<EPL, 9, WIN, false>, a, grid, threads, smem);
     }
 }
 
@@ -665,6 +677,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
         prof_begin(c, KID_CELLS);
         rc = PPM_OK;
         if (wst) {
+            CK(cudaMemsetAsync(c->d_pairs + 1, 0, sizeof(unsigned long long), c->stream));
             CellArgs W = A;
             W.nw = 16;
             dim3 gridw(c->nchunk, (g.n_phase + 15) / 16, nb * c->n_etile);

@@ -333,24 +333,34 @@ __device__ __forceinline__ void smem_check(const void* p, size_t bytes, const vo
 #define PPM_SMEM_CHECK(p, bytes) ((void)0)
 #endif
 
+// Node value of a pair at slice column n for the uniform-temperature kernels: the row's one (mu x logx) slice.
+struct SliceNode {
+    const double* srow;                  // slice row of the stencil's first mu node
+    int nx;
+    double v0, v1, v2, v3, qb;           // mu weights (pre-scaled by log2(10)) and log2(F_p T^3)
+    __device__ __forceinline__ double operator()(int n) const { return node_value(srow + n, nx, v0, v1, v2, v3, qb); }
+    __device__ __forceinline__ void check(int n0, int count, const double* sm) const
+    {
+        PPM_SMEM_CHECK(srow + n0, sizeof(double) * (3 * nx + count));
+        (void)n0; (void)count; (void)sm;
+    }
+};
+
 // ---- fused pass of a pair: node values -> interval coefficients.  Lane l holds nodes n0 .. n0+NPL-1, n0 = jlo-1 + NPL l;
 // interval c (nodes c, c+1) has window offset c - (jlo-1).  Out-of-table nodes read neighbouring shared memory: they only
-// feed window slots that no energy reads.  Node value = sum_mu v_mu S[mu][node] + qb.  Writes KA[0..KW) = (k0,k1),
-// KA[KW..2KW) = (k2,k3); both __syncwarp's are inside (the previous pair's readers are done / the new coefficients are
-// visible).
-template <int NPL>
-__device__ __forceinline__ void fused_pass(const double* __restrict__ srow, int nx, int jlo, int jhi, int lane, double v0,
-                                           double v1, double v2, double v3, double qb, int x_linedge, double2* KA,
+// feed window slots that no energy reads.  node(n) = the pair's value at slice column n (SliceNode; MapNode of
+// ppm_cells_map.cuh blends two log T node slices).  Writes KA[0..KW) = (a0,a1), KA[KW..2KW) = (a2,a3); both
+// __syncwarp's are inside (the previous pair's readers are done / the new coefficients are visible).
+template <int NPL, class NodeFn>
+__device__ __forceinline__ void fused_pass(const NodeFn& node, int nx, int jlo, int jhi, int lane, int x_linedge, double2* KA,
                                            const double* sm)
 {
     constexpr int KW = 32 * NPL;
     const int n0 = jlo - 1 + NPL * lane;
-    const double* sp0 = srow + n0;
-    PPM_SMEM_CHECK(sp0, sizeof(double) * (3 * nx + NPL));
-    (void)sm;
+    node.check(n0, NPL, sm);
     double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
 #pragma unroll
-    for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node_value(sp0 + jn, nx, v0, v1, v2, v3, qb);
+    for (int jn = 0; jn < NPL; ++jn) f[1 + jn] = node(n0 + jn);
     f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
     if (NPL == 1) {
         f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
@@ -375,7 +385,7 @@ __device__ __forceinline__ void fused_pass(const double* __restrict__ srow, int 
                 const int s = (c == 0) ? 0 : nx - 4;
                 double g[4];
 #pragma unroll
-                for (int m = 0; m < 4; ++m) g[m] = node_value(srow + s + m, nx, v0, v1, v2, v3, qb);
+                for (int m = 0; m < 4; ++m) g[m] = node(s + m);
                 double k0, k1, k2, k3;
                 cubic_coeffs(g[0], g[1], g[2], g[3], k0, k1, k2, k3);
                 const double d = (double)(c - 1 - s);               // Taylor shift: this interval is [1, 2) of its own t
@@ -483,6 +493,70 @@ __device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], c
     else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1, UNI>(g, acc, ec, KAq, q, s_top);
 }
 
+// Number of energy groups of a pair whose FIRST energy still lies inside the table (used when only PAIR_CLAMP_HI is set):
+// UG[i] = coordinate part of group i's first energy (a group without any energy holds 2^62).
+template <int NG>
+__device__ __forceinline__ int clamped_groups(long long pq, const long long* __restrict__ UG, long long s_top)
+{
+    int g = 0;
+#pragma unroll
+    for (int i = 0; i < NG; ++i) g += (pq + UG[i] <= s_top) ? 1 : 0;
+    return g;
+}
+
+// The energies of one pair (step B, part ii): KAq = the pair's coefficient window indexed by interval, q = its coordinate,
+// flg = its flags (bits 8.. = clamped_groups when only PAIR_CLAMP_HI is set), hdef = the lane's deferred sum.
+template <int KW, int EPL, bool UNI>
+__device__ __forceinline__ void pair_energies(double (&acc)[EPL], double& hdef, const EnergyCoord<EPL, UNI>& ec,
+                                              const double2* __restrict__ KAq, long long q, int flg, long long s_top, int lane,
+                                              const double* sm)
+{
+    (void)sm;
+    if (flg == 0) {
+        // every coordinate of the tile lies inside the table and every exponent is in range
+        long long s = ec.first(q);
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) {
+            PPM_SMEM_CHECK(KAq + (s >> 52), sizeof(double2));
+            PPM_SMEM_CHECK(KAq + (s >> 52) + KW, sizeof(double2));
+            acc[i] += triple_value<KW>(KAq, s);
+            s = ec.next(s, q, i);
+        }
+    } else if ((flg & 7) == PAIR_CLAMP_HI) {
+        // the upper energies lie beyond the top of the logx axis: the clamped coordinate (reading R13b) makes their term
+        // the pair's constant 2^y(s_top).  Groups g .. EPL-1 (g = flg >> 8) are clamped for every lane: the constant goes
+        // to lane g's deferred sum and is spread over acc[g ..] once, in the epilogue (spread_deferred).
+        const int g = flg >> 8;
+        if (g < EPL) {                                                          // (g == EPL: only the last group straddles the end)
+            const double vtop = triple_value<KW>(KAq, s_top);
+            if (lane == g) hdef += vtop;
+        }
+        dispatch_clamped_hi<KW, EPL, EPL, UNI>(g, acc, ec, KAq, q, s_top);
+    } else {
+        // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
+        // range-checked form
+        long long s = ec.first(q);
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) {
+            acc[i] += triple_value_checked<KW>(KAq, s, s_top);
+            s = ec.next(s, q, i);
+        }
+    }
+}
+
+// deferred constants of the clamped groups: acc[i] += sum over g <= i of lane g's hdef (inclusive scan over lanes)
+template <int EPL>
+__device__ __forceinline__ void spread_deferred(double (&acc)[EPL], double hdef, int lane)
+{
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const double up = __shfl_up_sync(0xffffffffu, hdef, d);
+        if (lane >= d) hdef += up;
+    }
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, i);
+}
+
 template <int EPL, int NPL, bool UNI>
 __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
@@ -582,12 +656,7 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 if (Fp != 0.0) {
                     pair_table_record(Fp, zp, mup, sp.log10kT, sp.log2T3, MUAX, A.nmu, A.mu_rule, nx, A.inv_h, A.x0_over_h,
                                       uef_first, uef_last, s_top, A.y_lo, A.y_hi, pq, pb, ww, info, flags);
-                    if (flags == PAIR_CLAMP_HI) {                               // groups whose first energy is inside the table
-                        int g = 0;
-#pragma unroll
-                        for (int i = 0; i < NG; ++i) g += (pq + UG[i] <= s_top) ? 1 : 0;
-                        flags |= g << 8;
-                    }
+                    if (flags == PAIR_CLAMP_HI) flags |= clamped_groups<NG>(pq, UG, s_top) << 8;
                 }
             }
             const unsigned valid = __ballot_sync(0xffffffffu, Fp != 0.0);
@@ -610,52 +679,15 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 const long long q = __double_as_longlong(r0.x);
                 const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                 const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
-                const double* srow = S + (inf & 0xFFFF);
-                fused_pass<NPL>(srow, nx, jlo, jhi, lane, v0, v1, v2, v3, qb, A.x_linedge, KA, sm);
+                const SliceNode node{S + (inf & 0xFFFF), nx, v0, v1, v2, v3, qb};
+                fused_pass<NPL>(node, nx, jlo, jhi, lane, A.x_linedge, KA, sm);
                 const double2* KAq = KA + (1 - jlo);
-                // ---- energies ----
-                if (flg == 0) {
-                    // every coordinate of the tile lies inside the table and every exponent is in range
-                    long long s = ec.first(q);
-#pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        PPM_SMEM_CHECK(KAq + (s >> 52), sizeof(double2));
-                        PPM_SMEM_CHECK(KAq + (s >> 52) + KW, sizeof(double2));
-                        acc[i] += triple_value<KW>(KAq, s);
-                        s = ec.next(s, q, i);
-                    }
-                } else if ((flg & 7) == PAIR_CLAMP_HI) {
-                    // the upper energies lie beyond the top of the logx axis: the clamped coordinate (reading R13b) makes
-                    // their term the pair's constant 2^y(s_top).  Groups g .. EPL-1 (g = flg >> 8) are clamped for every lane:
-                    // the constant goes to lane g's deferred sum and is spread over acc[g ..] once, in the epilogue.
-                    const int g = flg >> 8;
-                    if (g < NG) {                                               // (g == NG: only the last group straddles the end)
-                        const double vtop = triple_value<KW>(KAq, s_top);
-                        if (lane == g) hdef += vtop;
-                    }
-                    dispatch_clamped_hi<KW, EPL, EPL, UNI>(g, acc, ec, KAq, q, s_top);
-                } else {
-                    // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
-                    // range-checked form
-                    long long s = ec.first(q);
-#pragma unroll
-                    for (int i = 0; i < EPL; ++i) {
-                        acc[i] += triple_value_checked<KW>(KAq, s, s_top);
-                        s = ec.next(s, q, i);
-                    }
-                }
+                pair_energies<KW, EPL, UNI>(acc, hdef, ec, KAq, q, flg, s_top, lane, sm);
             }
         }
     }
     if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
-    // deferred constants of the clamped groups: acc[i] += sum over g <= i of lane g's hdef (inclusive scan over lanes)
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const double up = __shfl_up_sync(0xffffffffu, hdef, d);
-        if (lane >= d) hdef += up;
-    }
-#pragma unroll
-    for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, i);
+    spread_deferred<EPL>(acc, hdef, lane);
     if (kvalid) {
         double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
 #pragma unroll

@@ -120,7 +120,8 @@ __global__ void __launch_bounds__(512, 1) k_cells_lin(CellArgs A)
                 const long long q = __double_as_longlong(r0.x);
                 const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
                 const double* srow = S + (inf & 0xFFFF);
-                fused_pass<NPL>(srow, nx, jlo, jhi, lane, r1.x, r1.y, r2.x, r2.y, 0.0, A.x_linedge, KA, sm);
+                const SliceNode node{srow, nx, r1.x, r1.y, r2.x, r2.y, 0.0};
+                fused_pass<NPL>(node, nx, jlo, jhi, lane, A.x_linedge, KA, sm);
                 const double2* KAq = KA + (1 - jlo);
 #pragma unroll
                 for (int i = 0; i < EPL; ++i) {

@@ -11,8 +11,9 @@
 // interval is the lower node of the next: ping-pong, one new slice per step), and processes the row's cells of that
 // interval.  Two full-width FP64 slices take 178 KB (room for 8 warps only); the WIN variant cuts the slices to the
 // logx columns the interval's pairs can reach (map_window) and keeps 16 warps.
-// Everything per pair and per triple is k_cells_tab's scheme (fixed-point logx coordinate, fused shuffle pass to
-// per-interval monomial coefficients, Horner + degree-8 exp2), with T, kT and T^3 taken per cell.
+// Everything per pair and per triple is k_cells_tab's own code (pair_table_record, fused_pass with a node functor that
+// blends the two slices, pair_energies with the stepped coordinate and the deferred clamped groups), with T, kT and T^3
+// taken per cell.
 #pragma once
 #include "ppm_cells.cuh"
 
@@ -22,6 +23,21 @@ __device__ __forceinline__ double contract4(const double* __restrict__ sp0, int 
 {
     return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
 }
+
+// Node value of a pair in temperature-map mode: the mu stencil on the slices of the two log T nodes that bracket the
+// cell's temperature, blended with (1 - t, t), plus log2(F_p T^3).  `lo` / `hi` point at the stencil's first mu row of
+// the two slice buffers, already shifted so that column n of the table is element n.
+struct MapNode {
+    const double* lo;
+    const double* hi;
+    int stride;
+    double v0, v1, v2, v3, w0, w1, qb;
+    __device__ __forceinline__ double operator()(int n) const
+    {
+        return fma(w1, contract4(hi + n, stride, v0, v1, v2, v3), fma(w0, contract4(lo + n, stride, v0, v1, v2, v3), qb));
+    }
+    __device__ __forceinline__ void check(int, int, const double*) const {}
+};
 
 // logx node window [c_lo, c_hi] that bounds every pair of log T interval `it` of a row: u = (log10(z E / kT) - x0) / h
 // over z in [zlo, zhi] (template), E in [E_first, E_last] (energy tile, as fixed-point uef) and log T in the part of the
@@ -53,11 +69,13 @@ __device__ inline bool map_row_fits(const RowD& row, const double* __restrict__ 
 }
 
 // WIN = true: 16 warps, the two node slices hold only the window's columns (row stride A.wst); rows whose windows do not
-// fit are skipped (the WIN = false launch takes them).  WIN = false: 8 warps, full-width slices (row stride nx).
-template <int EPL, int NPL, bool WIN>
+// fit are skipped and counted in A.pairs[1] (the WIN = false launch takes them, and returns at once when there are none).
+// WIN = false: 8 warps, full-width slices (row stride nx).
+template <int EPL, int NPL, bool WIN, bool UNI>
 __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
+    if (!WIN && A.map_split && A.pairs[1] == 0ull) return;                      // every row was taken by the windowed launch
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int chunk = blockIdx.x, pg = blockIdx.y;
     const int b = blockIdx.z / A.n_etile, et = blockIdx.z % A.n_etile;
@@ -69,36 +87,42 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
     const int wst = WIN ? A.wst : nx;                                           // row stride of the slice buffers
     const int plane = A.nmu * wst;
     // shared layout (doubles): per warp { KA [KW], KB [KW], R0 (q, qb), R1 (v0, v1), R2 (v2, v3), R3 (1-t, t) [32] as
-    // double2, RI [32] int } | S0 [nmu][nx] | S1 [nmu][nx] | T [4][n1] | MUAX [nmu] | TAX [nT]
+    // double2, RI [32] int2 (info, flags) } | S0 [nmu][wst] | S1 [nmu][wst] | T [4][n1] | MUAX [nmu] | TAX [nT] | UG [16]
     constexpr int KW = 32 * NPL;
-    constexpr int WARP_DBL = 4 * KW + 4 * 64 + 16;
+    constexpr int WARP_DBL = 4 * KW + 4 * 64 + 32;
     double* wbase = sm + (size_t)w * WARP_DBL;
     double2* KA = reinterpret_cast<double2*>(wbase);
     double2* R0 = KA + 2 * KW;
     double2* R1 = R0 + 32;
     double2* R2 = R1 + 32;
     double2* R3 = R2 + 32;
-    int* RI = reinterpret_cast<int*>(R3 + 32);
+    int2* RI = reinterpret_cast<int2*>(R3 + 32);
     double* Sb0 = sm + (size_t)A.nw * WARP_DBL;
     double* Sb1 = Sb0 + plane;
     double* T = Sb1 + plane;
     double* MUAX = T + 4 * n1;
     double* TAX = MUAX + A.nmu;
+    long long* UG = reinterpret_cast<long long*>(TAX + A.nT);
+    constexpr int NG = EPL;
 
-    long long uef[EPL];
+    EnergyCoord<EPL, UNI> ec;
+    ec.init(A.uef, A.uef_step, e0, lane, A.nE);
     double acc[EPL];
 #pragma unroll
-    for (int i = 0; i < EPL; ++i) {
-        const int e = e0 + lane + 32 * i;
-        uef[i] = A.uef[e < A.nE ? e : A.nE - 1];
-        acc[i] = 0.0;
-    }
+    for (int i = 0; i < EPL; ++i) acc[i] = 0.0;
+    double hdef = 0.0;
     const long long uef_first = A.uef[imin_(e0, A.nE - 1)];
-    const long long uef_last = A.uef[imin_(e0 + 32 * EPL, A.nE) - 1];
+    const int e_last = imin_(e0 + 32 * EPL, A.nE) - 1;
+    const long long uef_last = UNI ? A.uef[e0 + ((e_last - e0) & 31)] + (long long)((e_last - e0) >> 5) * A.uef_step
+                                   : A.uef[e_last];
     const long long s_top = ((long long)(nx - 1) << 52) - 1;
     const double ue_first = (double)uef_first / kTwo52, ue_last = (double)uef_last / kTwo52;
     for (int i = threadIdx.x; i < A.nmu; i += blockDim.x) MUAX[i] = A.axmu[i];
     for (int i = threadIdx.x; i < A.nT; i += blockDim.x) TAX[i] = A.axT[i];
+    if (threadIdx.x < NG) {
+        const int ef = e0 + 32 * (int)threadIdx.x;
+        UG[threadIdx.x] = (ef < A.nE) ? (UNI ? A.uef[e0] + (long long)threadIdx.x * A.uef_step : A.uef[ef]) : (1ll << 62);
+    }
 
     const StarD& st = A.stars[b];
     const double phi_off = st.phi_off;
@@ -115,7 +139,10 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
         if (nact == 0 || !row.visible) continue;
         if (A.map_split) {                                                       // each row belongs to exactly one launch
             const bool fits = map_row_fits(row, A.axT, A.nT, A.inv_h, A.x0_over_h, ue_first, ue_last, nx, A.wst);
-            if (fits != WIN) continue;
+            if (fits != WIN) {
+                if (WIN && pg == 0 && et == 0 && threadIdx.x == 0) atomicAdd(A.pairs + 1, 1ull);
+                continue;
+            }
         }
         const SpotD& sp = A.spots[rid / A.n_theta];
         __syncthreads();
@@ -129,6 +156,11 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
         const double* MU = T + 3 * n1;
         const int* cl = A.cells + (size_t)rid * A.n_phi;
         const double* tcell = A.tmap + (size_t)rid * A.n_phi;
+        // the row's two log g nodes (strategy d: linear; axis_w4 puts the weights at stencil offsets o, o + 1)
+        int go = 0;
+        while (go < 2 && row.wg[go] == 0.0) ++go;
+        const double wga = row.wg[go], wgb = row.wg[go + 1];
+        const size_t gplane = (size_t)A.nmu * nx;
         int pos = 0;                                                             // next unprocessed entry of the sorted cell list
         int node0 = -1, node1 = -1;                                              // log T node held by slice buffer 0 / 1
         for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
@@ -143,22 +175,19 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                 if (!WIN && (buf ? node1 : node0) == node) continue;
                 if (buf) node1 = node; else node0 = node;
                 double* dst = buf ? Sb1 : Sb0;
-                const double* src = A.values + ((size_t)node * A.ng + row.bg) * ((size_t)A.nmu * nx);
+                const double* src = A.values + ((size_t)node * A.ng + row.bg + go) * gplane + (WIN ? c_lo : 0);
                 const int wcols = WIN ? c_hi - c_lo + 1 : nx;
-                for (int i = threadIdx.x; i < A.nmu * wcols; i += blockDim.x) {
-                    const int mu_i = i / wcols, col = i - mu_i * wcols;
-                    const size_t gi = (size_t)mu_i * nx + (WIN ? c_lo : 0) + col;
-                    double v = 0.0;
-#pragma unroll
-                    for (int gq = 0; gq < 4; ++gq)
-                        if (row.wg[gq] != 0.0) v = fma(row.wg[gq], __ldg(src + (size_t)gq * A.nmu * nx + gi), v);
-                    dst[mu_i * wst + col] = v;
+                // 128 consecutive threads walk the columns of one mu row (coalesced), blockDim / 128 rows per pass
+                for (int mu_i = threadIdx.x >> 7; mu_i < A.nmu; mu_i += blockDim.x >> 7) {
+                    const double* s0 = src + (size_t)mu_i * nx;
+                    for (int col = threadIdx.x & 127; col < wcols; col += 128)
+                        dst[mu_i * wst + col] = fma(wgb, __ldg(s0 + gplane + col), wga * __ldg(s0 + col));
                 }
             }
             __syncthreads();
             if (!kvalid) continue;
-            const double* Slo = pl ? Sb1 : Sb0;
-            const double* Shi = pl ? Sb0 : Sb1;
+            const double* Slo = (pl ? Sb1 : Sb0) - c_lo;                         // column n of the table is element n
+            const double* Shi = (pl ? Sb0 : Sb1) - c_lo;
             const double po0 = PO[0];
             // the row's list is sorted by log T interval (k_rows): the cells of interval `it` start at `pos`
             for (bool more = true; more;) {
@@ -167,7 +196,7 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                 double Fp = 0.0, pb = 0.0, tw = 0.0;
                 long long pq = 0;
                 double ww[4] = {0.0, 0.0, 0.0, 0.0};
-                int info = 0;
+                int info = 0, flags = 0;
                 const int entry = (idx < nact) ? cl[idx] : -1;
                 const bool mine = (entry >= 0) && ((entry >> 16) == it);
                 const int n_mine = __popc(__ballot_sync(0xffffffffu, mine));     // a prefix of the batch (sorted list)
@@ -182,11 +211,10 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                     double zp, mup;
                     template_interp(F, Z, PO, MU, A.n_fp, A.phase_order, phi_p, Fp, zp, mup);                  // Eq 46
                     if (!(Fp > 0.0)) Fp = 0.0;
-                    if (Fp != 0.0) {
-                        int flags;                                                  // T, kT, T^3 of this cell
-                        pair_table_record(Fp, zp, mup, log10kB + lT, 3.0 * lT * kLog2_10, MUAX, A.nmu, A.mu_rule, 1, A.inv_h,
-                                          A.x0_over_h, uef_first, uef_last, s_top, 0.0, 0.0, pq, pb, ww, info, flags);
-                        if (flags & (PAIR_CLAMP_LO | PAIR_CLAMP_HI)) info |= 0x8000;
+                    if (Fp != 0.0) {                                                 // T, kT, T^3 of this cell
+                        pair_table_record(Fp, zp, mup, log10kB + lT, 3.0 * lT * kLog2_10, MUAX, A.nmu, A.mu_rule, wst, A.inv_h,
+                                          A.x0_over_h, uef_first, uef_last, s_top, A.y_lo, A.y_hi, pq, pb, ww, info, flags);
+                        if (flags == PAIR_CLAMP_HI) flags |= clamped_groups<NG>(pq, UG, s_top) << 8;
                         tw = tt;
                     }
                 }
@@ -200,88 +228,25 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                     R1[slot] = make_double2(ww[0], ww[1]);
                     R2[slot] = make_double2(ww[2], ww[3]);
                     R3[slot] = make_double2(1.0 - tw, tw);
-                    RI[slot] = info;
+                    RI[slot] = make_int2(info, flags);
                 }
                 __syncwarp();
                 // ---- step B: walk the valid pairs ----
                 for (int pj = 0; pj < cnt; ++pj) {
                     const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj], r3 = R3[pj];
-                    const int inf = RI[pj];
+                    const int2 ri2 = RI[pj];
+                    const int inf = ri2.x;
                     const long long q = __double_as_longlong(r0.x);
-                    const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                     const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
-                    const int soff = (inf & 0x7FFF) * wst - c_lo + jlo - 1 + NPL * lane;
-                    const int n0 = jlo - 1 + NPL * lane;
-                    double f[NPL + 3];
-#pragma unroll
-                    for (int jn = 0; jn < NPL; ++jn)
-                        f[1 + jn] = fma(r3.y, contract4(Shi + soff + jn, wst, v0, v1, v2, v3),
-                                        fma(r3.x, contract4(Slo + soff + jn, wst, v0, v1, v2, v3), qb));
-                    f[0] = __shfl_up_sync(0xffffffffu, f[NPL], 1);
-                    if (NPL == 1) {
-                        f[2] = __shfl_down_sync(0xffffffffu, f[1], 1);
-                        f[3] = __shfl_down_sync(0xffffffffu, f[1], 2);
-                    } else {
-                        f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
-                        f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
-                    }
-                    double2 ka[NPL], kb[NPL];
-#pragma unroll
-                    for (int jn = 0; jn < NPL; ++jn)
-                        cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
-                    if (jlo == 0 || jhi == nx - 2) {      // strategy d: linear in the first / last interval of the axis
-#pragma unroll
-                        for (int jn = 0; jn < NPL; ++jn) {
-                            const int c = n0 + jn;
-                            if (c != 0 && c != nx - 2) continue;
-                            const double d = f[jn + 2] - f[jn + 1];             // y = f1 + d (t - 1)
-                            ka[jn] = make_double2(f[jn + 1] - d, d);
-                            kb[jn] = make_double2(0.0, 0.0);
-                        }
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int jn = 0; jn < NPL; ++jn) {
-                        KA[NPL * lane + jn] = ka[jn];
-                        KA[NPL * lane + jn + KW] = kb[jn];
-                    }
-                    __syncwarp();
-                    const double2* KAq = KA + (1 - jlo);
-                    if (!(inf & 0x8000)) {
-#pragma unroll
-                        for (int i = 0; i < EPL; ++i) {
-                            const long long s = q + uef[i];
-                            const int shi = (int)(s >> 32);
-                            const double2* kp = KAq + (shi >> 20);
-                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s);   // t = 1 + fraction (see cubic_coeffs)
-                            const double2 c01 = kp[0], c23 = kp[KW];
-                            const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
-                            const double r = y + kMagic;
-                            const int n = __double2loint(r);
-                            const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                            if (n >= -1000) acc[i] += val;
-                        }
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < EPL; ++i) {
-                            long long s = q + uef[i];
-                            s = s < 0 ? 0 : (s > s_top ? s_top : s);             // clamp to the table (reading R13b)
-                            const int shi = (int)(s >> 32);
-                            const double2* kp = KAq + (shi >> 20);
-                            const double tau = __hiloint2double(one_plus_frac_hi(shi), (int)s);   // t = 1 + fraction (see cubic_coeffs)
-                            const double2 c01 = kp[0], c23 = kp[KW];
-                            const double y = fma(fma(fma(c23.y, tau, c23.x), tau, c01.y), tau, c01.x);
-                            const double r = y + kMagic;
-                            const int n = __double2loint(r);
-                            const double val = exp2_frac_scaled(y - (r - kMagic), n);
-                            if (n >= -1000) acc[i] += val;
-                        }
-                    }
+                    const MapNode node{Slo + (inf & 0xFFFF), Shi + (inf & 0xFFFF), wst, r1.x, r1.y, r2.x, r2.y, r3.x, r3.y, r0.y};
+                    fused_pass<NPL>(node, nx, jlo, jhi, lane, 1, KA, sm);           // strategy d: linear first / last interval
+                    pair_energies<KW, EPL, UNI>(acc, hdef, ec, KA + (1 - jlo), q, ri2.y, s_top, lane, sm);
                 }
             }
         }
     }
     if (kvalid && et == 0 && lane == 0 && npairs) atomicAdd(A.pairs, (unsigned long long)npairs);
+    spread_deferred<EPL>(acc, hdef, lane);
     if (kvalid) {
         double* out = A.partial + (((size_t)b * A.nchunk + chunk) * A.n_phase + k) * A.nE;
 #pragma unroll
