@@ -575,7 +575,7 @@ static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, 
 // shared memory of k_cells_map with `nw` warps (ppm_cells_map.cuh layout)
 static size_t cells_map_smem(const ppm_ctx* c, int nw, int wst)
 {
-    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 4 * 64 + 32) + 2 * (size_t)c->nmu * wst +
+    return sizeof(double) * ((size_t)nw * (4 * 32 * c->npl + 5 * 64 + 32) + 2 * (size_t)c->nmu * wst +
                              4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT + 16);
 }
 

@@ -24,17 +24,27 @@ __device__ __forceinline__ double contract4(const double* __restrict__ sp0, int 
     return fma(v3, sp0[3 * nx], fma(v2, sp0[2 * nx], fma(v1, sp0[nx], v0 * sp0[0])));
 }
 
-// Node value of a pair in temperature-map mode: the mu stencil on the slices of the two log T nodes that bracket the
-// cell's temperature, blended with (1 - t, t), plus log2(F_p T^3).  `lo` / `hi` point at the stencil's first mu row of
-// the two slice buffers, already shifted so that column n of the table is element n.
+// Node value of a pair in temperature-map mode: the (log T, mu) stencil -- 2 x 4 weights (1 - t) v_mu, t v_mu, formed once
+// per pair in step A -- on the slices of the two log T nodes that bracket the cell's temperature, plus log2(F_p T^3).
+// `lo` / `hi` point at the stencil's first mu row of the two slice buffers, each shifted by its own first column so that
+// column n of the table is element n.
 struct MapNode {
     const double* lo;
     const double* hi;
     int stride;
-    double v0, v1, v2, v3, w0, w1, qb;
+    double a0, a1, a2, a3, b0, b1, b2, b3, qb;   // (1 - t) v_mu and t v_mu: the (log T, mu) stencil's eight weights
     __device__ __forceinline__ double operator()(int n) const
     {
-        return fma(w1, contract4(hi + n, stride, v0, v1, v2, v3), fma(w0, contract4(lo + n, stride, v0, v1, v2, v3), qb));
+        const double* pl = lo + n;
+        const double* ph = hi + n;
+        double f = fma(a0, pl[0], qb);
+        f = fma(b0, ph[0], f);
+        f = fma(a1, pl[stride], f);
+        f = fma(b1, ph[stride], f);
+        f = fma(a2, pl[2 * stride], f);
+        f = fma(b2, ph[2 * stride], f);
+        f = fma(a3, pl[3 * stride], f);
+        return fma(b3, ph[3 * stride], f);
     }
     __device__ __forceinline__ void check(int, int, const double*) const {}
 };
@@ -56,14 +66,31 @@ __device__ inline void map_window(const RowD& row, const double* __restrict__ ax
     c_hi = imin_(imax_((int)floor(fmin(u_hi, (double)nx + 4.0)) + 3, 0), nx - 1);
 }
 
-// does every interval of the row fit a window of `wst` columns?  (rows that do not are left to the full-width kernel)
+// Columns held by the slice of log T node it + 1 when it is staged as the UPPER node of interval `it`: the interval's
+// window, widened to the next interval's window when the row also has cells there -- that interval then finds its lower
+// node already in shared memory (one new slice per step instead of two).  [c_lo, c_hi] = the window of interval `it`.
+__device__ inline void map_upper_window(const RowD& row, const double* __restrict__ axT, int nT, int it, double inv_h,
+                                        double x0_over_h, double ue_first, double ue_last, int nx, int c_lo, int c_hi,
+                                        int& n_lo, int& n_hi)
+{
+    n_lo = c_lo; n_hi = c_hi;
+    if ((row.tmask >> (it + 1)) & 1ull) {
+        int a_lo, a_hi;
+        map_window(row, axT, nT, it + 1, inv_h, x0_over_h, ue_first, ue_last, nx, a_lo, a_hi);
+        n_lo = imin_(n_lo, a_lo); n_hi = imax_(n_hi, a_hi);
+    }
+}
+
+// does every node slice of the row fit a window of `wst` columns?  (rows that do not are left to the full-width kernel)
 __device__ inline bool map_row_fits(const RowD& row, const double* __restrict__ axT, int nT, double inv_h, double x0_over_h,
                                     double ue_first, double ue_last, int nx, int wst)
 {
     for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
-        int c_lo, c_hi;
-        map_window(row, axT, nT, __ffsll((long long)tm) - 1, inv_h, x0_over_h, ue_first, ue_last, nx, c_lo, c_hi);
-        if (c_hi - c_lo + 1 > wst) return false;
+        const int it = __ffsll((long long)tm) - 1;
+        int c_lo, c_hi, n_lo, n_hi;
+        map_window(row, axT, nT, it, inv_h, x0_over_h, ue_first, ue_last, nx, c_lo, c_hi);
+        map_upper_window(row, axT, nT, it, inv_h, x0_over_h, ue_first, ue_last, nx, c_lo, c_hi, n_lo, n_hi);
+        if (n_hi - n_lo + 1 > wst) return false;
     }
     return true;
 }
@@ -86,17 +113,18 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
     const int nx = A.nx;
     const int wst = WIN ? A.wst : nx;                                           // row stride of the slice buffers
     const int plane = A.nmu * wst;
-    // shared layout (doubles): per warp { KA [KW], KB [KW], R0 (q, qb), R1 (v0, v1), R2 (v2, v3), R3 (1-t, t) [32] as
-    // double2, RI [32] int2 (info, flags) } | S0 [nmu][wst] | S1 [nmu][wst] | T [4][n1] | MUAX [nmu] | TAX [nT] | UG [16]
+    // shared layout (doubles): per warp { KA [KW], KB [KW], R0 (q, qb), R1 (a0, a1), R2 (a2, a3), R3 (b0, b1), R4 (b2, b3) [32]
+    // as double2, RI [32] int2 (info, flags) } | S0 [nmu][wst] | S1 [nmu][wst] | T [4][n1] | MUAX [nmu] | TAX [nT] | UG [16]
     constexpr int KW = 32 * NPL;
-    constexpr int WARP_DBL = 4 * KW + 4 * 64 + 32;
+    constexpr int WARP_DBL = 4 * KW + 5 * 64 + 32;
     double* wbase = sm + (size_t)w * WARP_DBL;
     double2* KA = reinterpret_cast<double2*>(wbase);
     double2* R0 = KA + 2 * KW;
     double2* R1 = R0 + 32;
     double2* R2 = R1 + 32;
     double2* R3 = R2 + 32;
-    int2* RI = reinterpret_cast<int2*>(R3 + 32);
+    double2* R4 = R3 + 32;
+    int2* RI = reinterpret_cast<int2*>(R4 + 32);
     double* Sb0 = sm + (size_t)A.nw * WARP_DBL;
     double* Sb1 = Sb0 + plane;
     double* T = Sb1 + plane;
@@ -163,20 +191,25 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
         const size_t gplane = (size_t)A.nmu * nx;
         int pos = 0;                                                             // next unprocessed entry of the sorted cell list
         int node0 = -1, node1 = -1;                                              // log T node held by slice buffer 0 / 1
+        int off0 = 0, off1 = 0;                                                  // first table column held by buffer 0 / 1
         for (unsigned long long tm = row.tmask; tm; tm &= tm - 1) {
             const int it = __ffsll((long long)tm) - 1;                           // log T interval [it, it+1]
             int c_lo = 0, c_hi = nx - 1;
             if (WIN) map_window(row, A.axT, A.nT, it, A.inv_h, A.x0_over_h, ue_first, ue_last, nx, c_lo, c_hi);
-            const int pl = (!WIN && node1 == it) ? 1 : 0;                        // windowed buffers are interval-specific: no reuse
+            // the previous interval's upper node is this interval's lower node when the intervals are adjacent; its slice
+            // was staged wide enough for both (map_upper_window): ping-pong, one new slice per step
+            const int pl = (node1 == it) ? 1 : 0;
             __syncthreads();                                                     // readers of the previous interval are done
 #pragma unroll
             for (int h = 0; h < 2; ++h) {                                        // h = 0: lower node -> buffer pl; 1: upper -> 1 - pl
                 const int buf = h ? 1 - pl : pl, node = it + h;
-                if (!WIN && (buf ? node1 : node0) == node) continue;
-                if (buf) node1 = node; else node0 = node;
+                if ((buf ? node1 : node0) == node) continue;
+                int n_lo = c_lo, n_hi = c_hi;
+                if (WIN && h) map_upper_window(row, A.axT, A.nT, it, A.inv_h, A.x0_over_h, ue_first, ue_last, nx, c_lo, c_hi, n_lo, n_hi);
+                if (buf) { node1 = node; off1 = n_lo; } else { node0 = node; off0 = n_lo; }
                 double* dst = buf ? Sb1 : Sb0;
-                const double* src = A.values + ((size_t)node * A.ng + row.bg + go) * gplane + (WIN ? c_lo : 0);
-                const int wcols = WIN ? c_hi - c_lo + 1 : nx;
+                const double* src = A.values + ((size_t)node * A.ng + row.bg + go) * gplane + n_lo;
+                const int wcols = n_hi - n_lo + 1;
                 // 128 consecutive threads walk the columns of one mu row (coalesced), blockDim / 128 rows per pass
                 for (int mu_i = threadIdx.x >> 7; mu_i < A.nmu; mu_i += blockDim.x >> 7) {
                     const double* s0 = src + (size_t)mu_i * nx;
@@ -186,8 +219,8 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
             }
             __syncthreads();
             if (!kvalid) continue;
-            const double* Slo = (pl ? Sb1 : Sb0) - c_lo;                         // column n of the table is element n
-            const double* Shi = (pl ? Sb0 : Sb1) - c_lo;
+            const double* Slo = pl ? Sb1 - off1 : Sb0 - off0;                    // column n of the table is element n
+            const double* Shi = pl ? Sb0 - off0 : Sb1 - off1;
             const double po0 = PO[0];
             // the row's list is sorted by log T interval (k_rows): the cells of interval `it` start at `pos`
             for (bool more = true; more;) {
@@ -225,20 +258,22 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                 if (Fp != 0.0) {
                     const int slot = __popc(valid & ((1u << lane) - 1u));
                     R0[slot] = make_double2(__longlong_as_double(pq), pb);
-                    R1[slot] = make_double2(ww[0], ww[1]);
-                    R2[slot] = make_double2(ww[2], ww[3]);
-                    R3[slot] = make_double2(1.0 - tw, tw);
+                    const double tl = 1.0 - tw;
+                    R1[slot] = make_double2(tl * ww[0], tl * ww[1]);
+                    R2[slot] = make_double2(tl * ww[2], tl * ww[3]);
+                    R3[slot] = make_double2(tw * ww[0], tw * ww[1]);
+                    R4[slot] = make_double2(tw * ww[2], tw * ww[3]);
                     RI[slot] = make_int2(info, flags);
                 }
                 __syncwarp();
                 // ---- step B: walk the valid pairs ----
                 for (int pj = 0; pj < cnt; ++pj) {
-                    const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj], r3 = R3[pj];
+                    const double2 r0 = R0[pj], r1 = R1[pj], r2 = R2[pj], r3 = R3[pj], r4 = R4[pj];
                     const int2 ri2 = RI[pj];
                     const int inf = ri2.x;
                     const long long q = __double_as_longlong(r0.x);
                     const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
-                    const MapNode node{Slo + (inf & 0xFFFF), Shi + (inf & 0xFFFF), wst, r1.x, r1.y, r2.x, r2.y, r3.x, r3.y, r0.y};
+                    const MapNode node{Slo + (inf & 0xFFFF), Shi + (inf & 0xFFFF), wst, r1.x, r1.y, r2.x, r2.y, r3.x, r3.y, r4.x, r4.y, r0.y};
                     fused_pass<NPL>(node, nx, jlo, jhi, lane, 1, KA, sm);           // strategy d: linear first / last interval
                     pair_energies<KW, EPL, UNI>(acc, hdef, ec, KA + (1 - jlo), q, ri2.y, s_top, lane, sm);
                 }
