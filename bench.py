@@ -207,15 +207,23 @@ def cpu_baseline(conf, mode="sample"):
                               "sample": one["sample"]}}
 
 
+def _code_only(text):
+    """the source without comments and with white space collapsed: the hash follows the code, not its commentary"""
+    import re
+    text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+    text = re.sub(r"//[^\n]*", " ", text)
+    return " ".join(text.split())
+
+
 def kernel_source_hash():
     """sha256 (first 16 hex digits) of the sources that define the table cell kernels: a capture in ncu_captured.json
     is used only for the kernel build it was taken from."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2510_07764_b200", "csrc")
-    for f in ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh"):
-        with open(os.path.join(d, f), "rb") as fh:
-            h.update(fh.read())
+    for f in ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh"):
+        with open(os.path.join(d, f), "r") as fh:
+            h.update(_code_only(fh.read()).encode())
     return h.hexdigest()[:16]
 
 

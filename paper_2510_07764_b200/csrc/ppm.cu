@@ -20,6 +20,7 @@
 #include "ppm_cells32.cuh"
 #include "ppm_cells_lin.cuh"
 #include "ppm_cells_map.cuh"
+#include "ppm_cells_map4.cuh"
 #include "ppm_observe.cuh"
 #include "ppm_chain.cuh"
 
@@ -112,6 +113,7 @@ struct ppm_ctx {
     long long* d_uef = nullptr;                   // log10(E)/h in fixed point (2^-52 intervals)
     int npl = 1;                                  // nodes per lane of the table cell kernel's fused pass
     bool uniform_e = false;                       // log-uniform energy grid: the cell kernels step the coordinate (EnergyCoord)
+    int m4_epl = 0, m4_ntile = 0, m4_npl = 0, m4_nw = 0, m4_wst = 0;   // tiling of k_cells_map4 (0: does not fit)
     long long uef_step = 0;                       // 32 * the grid's step of uef
     std::vector<double> h_en;
     // atmosphere
@@ -204,6 +206,8 @@ extern "C" int ppm_destroy(ppm_ctx* c)
     delete c;
     return PPM_OK;
 }
+
+static void choose_map4_tiling(ppm_ctx* c, const std::vector<double>& ue);
 
 // dynamic shared memory of the table cell kernels for `npl` nodes per lane (ppm_cells.cuh / ppm_cells32.cuh layouts)
 static size_t cells_tab_smem(const ppm_ctx* c, int nmu, int nx, int npl)
@@ -448,6 +452,7 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
             }
             if (ok) { c->uniform_e = true; c->uef_step = step32; }
         }
+        choose_map4_tiling(c, ue);
     }
     CK(cudaStreamSynchronize(c->stream));
     c->have_atm = true;
@@ -579,6 +584,59 @@ static size_t cells_map_smem(const ppm_ctx* c, int nw, int wst)
                              4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT + 16);
 }
 
+// shared memory of k_cells_map4 with `nw` warps, `npl` nodes per lane and slices of `wst` columns (ppm_cells_map4.cuh layout)
+static size_t cells_map4_smem(const ppm_ctx* c, int nw, int npl, int wst)
+{
+    return sizeof(double) * ((size_t)nw * (4 * 32 * npl + 5 * 64 + 32) + 4 * (size_t)c->nmu * wst +
+                             4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT + 16);
+}
+
+// Tiling of k_cells_map4 (temperature maps under the cubic-in-log-T strategies): the most energies per lane, then the
+// most warps, for which four slices wide enough for a tile's window (+ 20 columns for the row's z range, the log T
+// interval and the stencil's reach) fit the 227 KB beside the warps' coefficient arrays.
+static void choose_map4_tiling(ppm_ctx* c, const std::vector<double>& ue)
+{
+    c->m4_epl = c->m4_ntile = c->m4_npl = c->m4_nw = c->m4_wst = 0;
+    const int nE = c->cfg.n_energy, need = (nE + 31) / 32;
+    const int epls[] = {10, 8, 5, 4, 2, 1};
+    int vbest = 10;
+    for (int v : epls) if (v >= need) vbest = v;
+    for (int v : epls) {
+        if (v > vbest) continue;
+        const int ntile = (nE + 32 * v - 1) / (32 * v);
+        int wmax = 1;
+        for (int t = 0; t < ntile; ++t) {
+            const int ea = t * 32 * v, eb = std::min(nE, ea + 32 * v) - 1;
+            wmax = std::max(wmax, std::min(c->nx - 1, (int)std::floor(ue[eb] - ue[ea]) + 3));
+        }
+        int npl = 1;
+        while (32 * npl - 3 < wmax) npl += 2;
+        if (npl > 3) continue;
+        for (int nw : {16, 8, 4}) {
+            if (nw > std::max(4, c->cfg.n_phase)) continue;
+            const long budget = 227 * 1024 / 8 - (long)(cells_map4_smem(c, nw, npl, 0) / 8);
+            const int wst = (int)std::min<long>(c->nx, budget > 0 ? budget / (4 * c->nmu) : 0);
+            if (wst >= std::min(c->nx, wmax + 20)) {
+                c->m4_epl = v; c->m4_ntile = ntile; c->m4_npl = npl; c->m4_nw = nw; c->m4_wst = wst;
+                return;
+            }
+        }
+    }
+}
+
+template <int EPL>
+static int dispatch_cells_map4(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+    if (c->m4_npl == 1) {
+        CK(cudaFuncSetAttribute(k_cells_map4<EPL, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_cells_map4<EPL, 1><<<grid, threads, smem, c->stream>>>(a, c->d_stars);
+    } else {
+        CK(cudaFuncSetAttribute(k_cells_map4<EPL, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_cells_map4<EPL, 3><<<grid, threads, smem, c->stream>>>(a, c->d_stars);
+    }
+    return PPM_OK;
+}
+
 template <int EPL, bool WIN>
 static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
@@ -652,13 +710,30 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     const bool cubic_all = g.emission == PPM_EMISSION_TABLE_CUBIC || g.emission == PPM_EMISSION_TABLE_CUBIC_CLIP;   // a, b
     A.mu_rule = cubic_all ? AX_CUBIC_SHIFT : AX_MU_PROTECTED;
     A.x_linedge = cubic_all ? 0 : 1;
+    A.t_rule = tg_rule(g.emission);
     A.clip = (g.interp_domain == 1 && g.emission == PPM_EMISSION_TABLE_CUBIC_CLIP) ? 1 : 0;
     A.nchunk = c->nchunk; A.rows_per_chunk = c->rows_per_chunk; A.nw = c->nw; A.n_etile = c->n_etile; A.mesh = g.mesh; A.beaming = g.beaming;
     A.phase_order = g.phase_interp == 3 ? 3 : 1; A.y_lo = c->y_lo; A.y_hi = c->y_hi;
     const size_t smem = table ? cells_tab_smem(c, c->nmu, c->nx, c->npl) : sizeof(double) * 4 * (size_t)(c->n_fp + 1);
     if (smem > 227 * 1024) { set_err("cell kernel needs %zu bytes of shared memory (> 227 KB)", smem); return PPM_ERR_ARG; }
     int rc;
-    if (tmap_dev) {
+    if (tmap_dev && g.emission != PPM_EMISSION_TABLE_MIXED) {
+        // temperature-map mode under the strategies that are cubic in log T: four windowed node slices, own energy tiling
+        A.tmap = tmap_dev; A.values = c->d_values; A.axT = c->d_axT; A.nT = c->nT; A.ng = c->ng;
+        A.nw = c->m4_nw; A.n_etile = c->m4_ntile; A.wst = c->m4_wst; A.map_split = 0; A.uniform_e = 0;
+        dim3 grid(c->nchunk, (g.n_phase + c->m4_nw - 1) / c->m4_nw, nb * c->m4_ntile);
+        const size_t sm4 = cells_map4_smem(c, c->m4_nw, c->m4_npl, c->m4_wst);
+        prof_begin(c, KID_CELLS);
+        switch (c->m4_epl) {
+        case 1:  rc = dispatch_cells_map4<1>(c, A, grid, c->m4_nw * 32, sm4); break;
+        case 2:  rc = dispatch_cells_map4<2>(c, A, grid, c->m4_nw * 32, sm4); break;
+        case 4:  rc = dispatch_cells_map4<4>(c, A, grid, c->m4_nw * 32, sm4); break;
+        case 5:  rc = dispatch_cells_map4<5>(c, A, grid, c->m4_nw * 32, sm4); break;
+        case 8:  rc = dispatch_cells_map4<8>(c, A, grid, c->m4_nw * 32, sm4); break;
+        default: rc = dispatch_cells_map4<10>(c, A, grid, c->m4_nw * 32, sm4); break;
+        }
+        c->launches += 1;
+    } else if (tmap_dev) {
         // temperature-map mode: two FP64 log T node slices in shared memory.  Full-width slices leave room for 8 warps;
         // slices cut to the logx columns a row's interval can reach (wst columns) leave room for 16.  Both kernels are
         // launched, each row is taken by the windowed one if all its intervals fit wst columns, else by the full-width one.
@@ -752,11 +827,15 @@ extern "C" int ppm_evaluate_map(ppm_ctx* c, const double* params_dev, const doub
     if (B == 0) return PPM_OK;
     ARG(params_dev && logT_map_dev && flux_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
-    if (c->cfg.emission != PPM_EMISSION_TABLE_MIXED || c->cfg.precision != 0 || c->cfg.interp_domain != 0) {
-        set_err("temperature maps need emission = 2 (linear in log T), precision = 0 and interp_domain = 0"); return PPM_ERR_STATE;
+    if (c->cfg.emission == PPM_EMISSION_BLACKBODY || c->cfg.precision != 0 || c->cfg.interp_domain != 0) {
+        set_err("temperature maps need table emission (1-4), precision = 0 and interp_domain = 0"); return PPM_ERR_STATE;
     }
     if (!c->have_atm) { set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE; }
     if (c->nT > 64) { set_err("temperature maps support at most 64 log T nodes"); return PPM_ERR_STATE; }
+    if (c->cfg.emission != PPM_EMISSION_TABLE_MIXED && !c->m4_epl) {
+        set_err("temperature maps under strategies a-c: four log T node slices do not fit shared memory for this table / energy grid");
+        return PPM_ERR_STATE;
+    }
     CK(cudaSetDevice(c->cfg.device));
     const size_t fstride = (size_t)c->cfg.n_phase * c->cfg.n_energy;
     const size_t mstride = (size_t)c->RT * c->cfg.n_phi;

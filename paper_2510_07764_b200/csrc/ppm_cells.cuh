@@ -29,6 +29,7 @@ struct CellArgs {
     double x0_over_h, inv_h;
     int nb, RT, n_spots, n_theta, n_phi, n_phase, n_fp, nE;
     int nmu, nx, mu_rule, x_linedge;
+    int t_rule;              // temperature-map mode under strategies a-c (k_cells_map4): AxisRule of the log T axis
     int nchunk, rows_per_chunk, nw, n_etile, mesh;
     int beaming;             // blackbody only: 0 isotropic, 1 cos^2(sigma'), 2 sin^2(sigma')
     int clip;                // intensity-domain interpolation (k_cells_lin): 1 = strategy b, negative intensities -> 0
@@ -267,18 +268,18 @@ __global__ void __launch_bounds__(512, 1) k_cells_bb(CellArgs A)
 // ownership as k_cells above (output-stationary accumulators, no atomics); what differs is how a
 // (cell, phase) pair is turned into its energies' terms:
 //  * logx coordinate in fixed point.  u = (log10(z_p E_e / kT) - x0)/h = u_pair + u_e is carried as a
-//    64-bit integer in units of 2^-52 intervals: s = q_pair + uef[e] (two integer adds).  The interval
-//    index is s >> 52 and the fraction, OR-ed under the exponent of 1.0, gives 1 + frac directly as a
-//    double: tau = (1 + frac) - 1.5 is the offset from the interval midpoint -- 1 DADD instead of the
-//    4 of a floating-point round-and-subtract, and the window below is found with the same integers.
+//    64-bit integer in units of 2^-52 intervals: s = q_pair + uef[e] (two integer adds; on log-uniform energy
+//    grids the lane steps s from one energy group to the next by one warp-uniform constant, EnergyCoord).  The
+//    interval index is s >> 52 and the fraction, OR-ed under the exponent of 1.0, gives t = 1 + frac directly
+//    as a double -- no floating-point round-and-subtract -- and the window below is found with the same integers.
 //  * one fused pass per pair over the window of logx intervals its energies touch: lane l contracts
 //    the mu stencil at NPL consecutive nodes (4 loads + 4 FMA each, slice rows in shared memory),
 //    takes the three neighbouring node values from lanes l-1 / l+1 by shuffle, and writes the
-//    monomial coefficients k0..k3 (in tau) of its NPL intervals -- cubic Lagrange on the 4 surrounding
-//    nodes; linear (strategy d) or the inward-shifted stencil (strategy a) in the first / last
-//    interval of the axis -- pre-scaled by log2(10), with log2(F_p T^3) added to k0.  NPL is odd so that
-//    the lanes' 8- and 16-byte accesses at stride NPL fall in distinct banks.
-//  * per triple: 2 x LDS.128 (k0..k3), Horner (3 DFMA), exp2 (3 DADD + 8 DFMA), accumulate (1 DADD).
+//    monomial coefficients a0..a3 in t (forward differences, cubic_coeffs) of its NPL intervals -- cubic
+//    Lagrange on the 4 surrounding nodes; linear (strategies c, d) or the inward-shifted stencil (strategies
+//    a, b) in the first / last interval of the axis -- pre-scaled by log2(10), with log2(F_p T^3) in a0.  NPL is
+//    odd so that the lanes' 8- and 16-byte accesses at stride NPL fall in distinct banks.
+//  * per triple: 2 x LDS.128 (a0..a3), Horner in t (3 DFMA), exp2 (3 DADD + 8 DFMA), accumulate (1 DADD).
 // The division by E_e of Eq 47 is the same for every term of a bin: applied once in the epilogue.
 // ------------------------------------------------------------------------------------------------
 constexpr double kTwo52 = 4503599627370496.0;

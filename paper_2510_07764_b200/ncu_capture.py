@@ -15,7 +15,7 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 JSON_PATH = os.path.join(HERE, "ncu_captured.json")
-HASHED = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh")
+HASHED = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh")
 
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
         "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "s": 1.0, "usecond": 1e-6, "nsecond": 1e-9, "msecond": 1e-3, "second": 1.0}
@@ -50,11 +50,19 @@ WANT = {
 }
 
 
+def _code_only(text):
+    """the source without comments and with white space collapsed (same rule as bench.py)"""
+    import re
+    text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+    text = re.sub(r"//[^\n]*", " ", text)
+    return " ".join(text.split())
+
+
 def source_hash():
     h = hashlib.sha256()
     for f in HASHED:
-        with open(os.path.join(HERE, "csrc", f), "rb") as fh:
-            h.update(fh.read())
+        with open(os.path.join(HERE, "csrc", f), "r") as fh:
+            h.update(_code_only(fh.read()).encode())
     return h.hexdigest()[:16]
 
 

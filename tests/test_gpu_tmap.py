@@ -82,14 +82,74 @@ def test_constant_map_equals_uniform_evaluate_and_batch_of_maps():
     assert np.all(st3 == 0) and np.all(g3 == 0.0)
 
 
-def test_map_mode_needs_strategy_d():
+def test_map_mode_needs_table_emission_and_fp64():
     import paper_2510_07764_b200 as ppm
     import torch
-    conf = gen.config_c2(n_cells=8, n_phase=8, n_energy=8)                       # emission = 1
+    conf = gen.config_c1()                                                      # closed-form blackbody: no table to map onto
     ctx = make_ctx(conf)
-    tm = torch.zeros((1, 1, 8, 8), dtype=torch.float64, device="cuda")
+    cfg = conf["cfg"]
+    tm = torch.full((1, cfg["n_spots"], cfg["n_theta"], cfg["n_phi"]), 6.0, dtype=torch.float64, device="cuda")
     with pytest.raises(ppm.PPMError):
         ctx.evaluate_map(torch.as_tensor(conf["params"], device="cuda"), tm)
+    conf = gen.config_c2(n_cells=8, n_phase=8, n_energy=8)
+    ctx = make_ctx(conf, precision=1)
+    tm = torch.full((1, 1, 8, 8), 6.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(ppm.PPMError):
+        ctx.evaluate_map(torch.as_tensor(conf["params"], device="cuda"), tm)
+
+
+@pytest.mark.parametrize("emission", [1, 3, 4])
+@pytest.mark.parametrize("mesh,n_energy", [(0, 70), (1, 70), (0, 300)])
+def test_cubic_in_log_T_strategies_match_oracle(emission, mesh, n_energy):
+    """Temperature maps under strategies a, c and b: cubic Lagrange in log T -- four node slices per
+    interval, stencil shifted inward (a, b) or linear (c) in the first / last log T interval -- on smooth seeded maps that
+    reach both ends of the log T axis; 300 energies run as two energy tiles of five energies per lane."""
+    conf = gen.config_c3(n_cells=28, n_phase=21, n_energy=n_energy)
+    conf["cfg"] = dict(conf["cfg"], emission=emission)
+    if n_energy == 300:
+        conf["energies"] = gen.logspace(0.2, 12.0, 300)
+    if mesh:
+        nside = 16
+        conf["cfg"] = dict(conf["cfg"], n_theta=4 * nside - 1, n_phi=4 * nside, mesh=1)
+    rng = np.random.default_rng(300 + 10 * emission + mesh)
+    tmap = _smooth_map(conf["cfg"], rng, lo=5.12, hi=6.78, holes=0.08)
+    g, st, ctx = _gpu_map(conf, tmap[None])
+    ref, so = o.evaluate(conf["cfg"], conf["energies"], conf["params"][0], oracle_atm(), tmap=tmap)
+    assert st[0] == 0 and so == 0 and ref.max() > 0
+    assert max_rel_err(g[0], ref) <= TOL
+
+
+def test_cubic_map_constant_equals_uniform_and_window_status():
+    """A constant map reproduces the uniform-temperature evaluate of the same strategy; temperatures inside the axis's
+    clamp range but outside the axis still work (own kT, clamped table coordinate); a row whose window exceeds the four
+    slice buffers gives PPM_STATUS_MAP_WINDOW and a NaN flux for that vector only."""
+    import torch
+    conf = gen.config_c5(n_vec=2, n_cells=20, n_phase=12, n_energy=40)
+    conf["cfg"] = dict(conf["cfg"], emission=1)
+    ctx = make_ctx(conf)
+    p = torch.as_tensor(conf["params"], device="cuda")
+    f_uni, _ = ctx.evaluate(p)
+    cfg = conf["cfg"]
+    tmap = np.empty((2, 2, cfg["n_theta"], cfg["n_phi"]))
+    for b in range(2):
+        tmap[b, 0], tmap[b, 1] = conf["params"][b, 8 + 3], conf["params"][b, 16 + 3]
+    g, st, _ = _gpu_map(conf, tmap, ctx)
+    fu = f_uni.cpu().numpy()
+    assert np.all(st == 0)
+    for b in range(2):
+        assert max_rel_err(g[b], fu[b]) <= 1e-11
+    tmap2 = tmap.copy()
+    tmap2[:, 0] = 5.02                                                           # just outside the axis at both ends
+    tmap2[:, 1] = 6.87
+    g2, st2, _ = _gpu_map(conf, tmap2, ctx)
+    ref, _ = o.evaluate(cfg, conf["energies"], conf["params"][1], oracle_atm(), tmap=tmap2[1])
+    assert np.all(st2 == 0) and max_rel_err(g2[1], ref) <= TOL
+    tmap3 = tmap.copy()
+    tmap3[1, 0, 3:6, ::2] = 9.0                                                  # 2.2 dex above the axis: the last interval's window
+                                                                                 # runs from column 0 to its own top, > 130 columns
+    g3, st3, _ = _gpu_map(conf, tmap3, ctx)
+    assert st3[0] == 0 and max_rel_err(g3[0], fu[0]) <= 1e-11
+    assert st3[1] == 8 and np.all(np.isnan(g3[1]))
 
 
 def test_rows_split_between_the_windowed_and_the_full_width_launch():
