@@ -13,7 +13,7 @@ CSRC = os.path.join(_HERE, "csrc")
 # kernel is checked against the block's allocation and traps outside it); it lives beside the product library.
 BOUNDS = os.environ.get("PPM_BOUNDS", "") not in ("", "0")
 LIB = os.path.join(_HERE, "libppm_b200_bounds.so" if BOUNDS else "libppm_b200.so")
-NVCC_FLAGS = ["-O3", "-std=c++17", "-split-compile", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
 

@@ -441,7 +441,7 @@ __device__ __forceinline__ double triple_value_checked(const double2* __restrict
 //  and the 2 EPL registers become 2.  The host takes this path only when every energy's own uef differs from that
 //  affine form by <= 256 units of 2^-52 intervals (5.7e-14 of a table interval: a relative change of the energy of 2.6e-15,
 //  ~ 12 ulp of a double; worst-case effect on a term 2.6e-13, the seeded grids deviate by <= 105 units) and when only the
-//  last group of a tile is ragged; a lane whose last energy does not exist re-evaluates its previous one (Dlast = 0; the
+//  last group of a tile is ragged; a lane whose last energy does not exist evaluates the tile's last real one (the
 //  result is never stored).
 template <int EPL, bool UNI>
 struct EnergyCoord {
@@ -452,7 +452,11 @@ struct EnergyCoord {
         if constexpr (UNI) {
             u[0] = uef[imin_(e0 + lane, nE - 1)];
             D = step;
-            Dlast = (e0 + lane + 32 * (EPL - 1) < nE) ? step : 0;
+            // a lane without a last energy sits on the tile's last real energy (one address for all such lanes: a
+            // broadcast, no bank conflict against the real lanes of its quarter-warp)
+            const int e_last = imin_(e0 + 32 * EPL, nE) - 1;
+            const long long last = uef[e0 + ((e_last - e0) & 31)] + (long long)((e_last - e0) >> 5) * step;
+            Dlast = (e0 + lane + 32 * (EPL - 1) < nE) ? step : last - (u[0] + (long long)(EPL - 2) * step);
         } else {
 #pragma unroll
             for (int i = 0; i < EPL; ++i) u[i] = uef[imin_(e0 + lane + 32 * i, nE - 1)];

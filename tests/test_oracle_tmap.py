@@ -14,13 +14,14 @@ def atm():
     return o.Atmosphere(*gen.synthetic_atmosphere())
 
 
-def _conf():
+def _conf(emission=2):
     c = gen.config_c3(n_cells=14, n_phase=10, n_energy=12)
-    return c["cfg"], c["energies"], c["params"][0]
+    return dict(c["cfg"], emission=emission), c["energies"], c["params"][0]
 
 
-def test_constant_map_equals_uniform_spot(atm):
-    cfg, E, p = _conf()
+@pytest.mark.parametrize("emission", [2, 1, 3])                     # strategies d, a, c: linear / cubic / cubic-linedge in log T
+def test_constant_map_equals_uniform_spot(atm, emission):
+    cfg, E, p = _conf(emission)
     f0, _ = o.evaluate(cfg, E, p, atm)
     tm = np.empty((2, 14, 14))
     tm[0], tm[1] = p[8 + 3], p[16 + 3]
@@ -46,14 +47,15 @@ def test_disjoint_maps_add_and_nan_cells_do_not_emit(atm):
     assert np.all(fn == 0)
 
 
-def test_two_temperature_map_on_healpix_equals_two_masked_spots(atm):
+@pytest.mark.parametrize("emission", [2, 1, 3])
+def test_two_temperature_map_on_healpix_equals_two_masked_spots(atm, emission):
     """Inner cap at T1 + surrounding ring at T2.  As spots: a cap (zeta = 0.15) and a cap (zeta = 0.4) with that inner
     cap omitted; as a map: one spot (zeta = 0.4) whose pixels carry T1 inside the inner cap and T2 outside."""
     nside = 12
     E = gen.logspace(0.2, 8.0, 10)
     th, ph = 1.1, 0.7
     T1, T2 = 6.35, 5.95
-    base = dict(n_theta=4 * nside - 1, n_phi=4 * nside, n_phase=8, n_fp=192, emission=2, oblate=1, mesh=1)
+    base = dict(n_theta=4 * nside - 1, n_phi=4 * nside, n_phase=8, n_fp=192, emission=emission, oblate=1, mesh=1)
     p2 = gen.pack_params(1.4, 12.0, 300.0, 0.5, 0.2, spots=[(th, ph, 0.15, T1), (th, ph, 0.4, T2, th, ph, 0.15)])
     f_spots, st = o.evaluate(dict(base, n_spots=2), E, p2, atm)
     inner = o.spot_mask_healpix(o.spot(th, ph, 0.15, T1), nside).astype(bool)
