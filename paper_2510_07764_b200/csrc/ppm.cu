@@ -21,7 +21,6 @@
 #include "ppm_cells_lin.cuh"
 #include "ppm_cells_map.cuh"
 #include "ppm_cells_map4.cuh"
-#include "ppm_cells_yx.cuh"
 #include "ppm_observe.cuh"
 #include "ppm_chain.cuh"
 
@@ -116,9 +115,6 @@ struct ppm_ctx {
     bool uniform_e = false;                       // log-uniform energy grid: the cell kernels step the coordinate (EnergyCoord)
     int m4_epl = 0, m4_ntile = 0, m4_npl = 0, m4_nw = 0, m4_wst = 0;   // tiling of k_cells_map4 (0: does not fit)
     long long uef_step = 0;                       // 32 * the grid's step of uef
-    long long uef_step1 = 0;                      // the grid's step of uef
-    int kmax = 0;                                 // most energies one table interval can hold
-    bool use_yx = false;                          // k_cells_yx instead of k_cells_tab (uniform grid, kmax <= 4, fits)
     std::vector<double> h_en;
     // atmosphere
     bool have_atm = false;
@@ -212,7 +208,6 @@ extern "C" int ppm_destroy(ppm_ctx* c)
 }
 
 static void choose_map4_tiling(ppm_ctx* c, const std::vector<double>& ue);
-static size_t cells_yx_smem(const ppm_ctx* c, int nmu, int nx);
 
 // dynamic shared memory of the table cell kernels for `npl` nodes per lane (ppm_cells.cuh / ppm_cells32.cuh layouts)
 static size_t cells_tab_smem(const ppm_ctx* c, int nmu, int nx, int npl)
@@ -442,28 +437,20 @@ extern "C" int ppm_load_atmosphere(ppm_ctx* c, const double* logT, int nT, const
         // Log-uniform energy grid?  Then energy e0 + lane + 32 i of a tile is evaluated at uef[e0 + lane] + i * step32 (see
         // EnergyCoord in ppm_cells.cuh).  Taken only if that affine form is within 256 units of 2^-52 table intervals of
         // every energy's own coordinate and only the last group of every tile is ragged.
-        c->uniform_e = false; c->uef_step = 0; c->uef_step1 = 0; c->kmax = 0; c->use_yx = false;
+        c->uniform_e = false; c->uef_step = 0;
         const int nE = c->cfg.n_energy;
         if (nE > 32 && c->epl >= 2) {
-            const long long step1 = llrintl((long double)(uef[nE - 1] - uef[0]) / (long double)(nE - 1));
-            const long long step32 = 32 * step1;
-            bool ok = step1 > 0, ok_affine = step1 > 0;
+            const long long step32 = llrintl(32.0L * (long double)(uef[nE - 1] - uef[0]) / (long double)(nE - 1));
+            bool ok = step32 > 0;
             for (int t = 0; t < c->n_etile && ok; ++t) {
                 const int ea = t * 32 * c->epl, nt = std::min(nE, ea + 32 * c->epl) - ea;
                 if (nt <= 32 * (c->epl - 1)) ok = false;            // more than the last group would be ragged
                 for (int k = 0; k < nt && ok; ++k) {
                     const long long dev = uef[ea + k] - (uef[ea + (k & 31)] + (long long)(k >> 5) * step32);
                     if (dev > 256 || dev < -256) ok = false;
-                    const long long dev1 = uef[ea + k] - (uef[ea] + (long long)k * step1);      // k_cells_yx's form
-                    if (dev1 > 256 || dev1 < -256) ok_affine = false;
                 }
             }
-            if (ok) {
-                c->uniform_e = true; c->uef_step = step32; c->uef_step1 = step1;
-                c->kmax = (int)((1ll << 52) / step1) + 1;
-                c->use_yx = ok_affine && c->kmax <= 4 && c->cfg.precision == 0 &&
-                            cells_yx_smem(c, nmu, nx) <= 227 * 1024;
-            }
+            if (ok) { c->uniform_e = true; c->uef_step = step32; }
         }
         choose_map4_tiling(c, ue);
     }
@@ -519,25 +506,6 @@ static int launch_cells(ppm_ctx* c, K kernel, const CellArgs& a, dim3 grid, int 
     return PPM_OK;
 }
 
-// dynamic shared memory of k_cells_yx (ppm_cells_yx.cuh layout)
-static size_t cells_yx_smem(const ppm_ctx* c, int nmu, int nx)
-{
-    return sizeof(double) * ((size_t)nmu * nx + 4 * (size_t)(c->n_fp + 1) + nmu + 16 +
-                             (size_t)c->nw * (2 * 32 * c->epl + 3 * 64 + 32));
-}
-
-template <int EPL>
-static int dispatch_cells_yx(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_yx<EPL, 1>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_yx<EPL, 3>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_yx<EPL, 5>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_yx<EPL, 7>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_yx<EPL, 9>, a, grid, threads, smem);
-    }
-}
-
 template <int EPL>
 static int dispatch_cells_tab32(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
@@ -568,8 +536,6 @@ static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int thre
     if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
     if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
     if constexpr (EPL >= 2) {
-        if (a.uniform_e && c->use_yx && getenv("PPM_YX"))
-            return dispatch_cells_yx<EPL>(c, a, grid, threads, cells_yx_smem(c, c->nmu, c->nx));
         if (a.uniform_e) {
             switch (c->npl) {
             case 1:  return launch_cells(c, k_cells_tab<EPL, 1, true>, a, grid, threads, smem);
@@ -736,7 +702,6 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
     A.stars = c->d_stars; A.spots = c->d_spots; A.rows = c->d_rows; A.cells = c->d_cells; A.tmpl = c->d_tmpl;
     A.slices = c->d_slices; A.axmu = c->d_axmu; A.uef = c->d_uef; A.en = c->d_en;
     A.uniform_e = (table && c->uniform_e) ? 1 : 0; A.uef_step = c->uef_step;
-    A.uef_step1 = c->uef_step1; A.inv_step1 = c->uef_step1 ? 1.0 / (double)c->uef_step1 : 0.0; A.kmax = c->kmax;
     A.partial = c->d_partial; A.pairs = c->d_pairs;
     A.x0_over_h = table ? c->x0 / c->hx : 0.0; A.inv_h = table ? 1.0 / c->hx : 0.0;
     A.nb = nb; A.RT = c->RT; A.n_spots = g.n_spots; A.n_theta = g.n_theta; A.n_phi = g.n_phi; A.n_phase = g.n_phase;

@@ -16,10 +16,7 @@ struct CellArgs {
     const long long* uef;    // [nE]: round(log10(E_e) / h * 2^52): energy part of the logx coordinate in fixed point
                              //       (h = logx spacing; units of 2^-52 table intervals)
     long long uef_step;      // log-uniform energy grids (uniform_e = 1): 32 * the grid's constant step of uef (see EnergyCoord)
-    long long uef_step1;     // the step itself (k_cells_yx: energy k of a tile sits at uef[e0] + k * uef_step1)
-    double inv_step1;        // 1 / uef_step1
     int uniform_e;
-    int kmax;                // k_cells_yx: most energies that one table interval can hold (<= 4)
     const double* en;        // [nE]: E_e (keV)
     double* partial;         // [nb][nchunk][n_phase][nE]
     const double* tmap;      // temperature-map mode: [rows][n_phi] log10 T per cell
@@ -356,9 +353,10 @@ struct SliceNode {
 // ppm_cells_map.cuh blends two log T node slices).  Writes KA[0..KW) = (a0,a1), KA[KW..2KW) = (a2,a3); both
 // __syncwarp's are inside (the previous pair's readers are done / the new coefficients are visible).
 template <int NPL, class NodeFn>
-__device__ __forceinline__ void interval_coeffs(const NodeFn& node, int nx, int jlo, int jhi, int lane, int x_linedge,
-                                                double2 (&ka)[NPL], double2 (&kb)[NPL], const double* sm)
+__device__ __forceinline__ void fused_pass(const NodeFn& node, int nx, int jlo, int jhi, int lane, int x_linedge, double2* KA,
+                                           const double* sm)
 {
+    constexpr int KW = 32 * NPL;
     const int n0 = jlo - 1 + NPL * lane;
     node.check(n0, NPL, sm);
     double f[NPL + 3];                    // f[1+j] = node n0+j; f[0] = node n0-1; f[NPL+1], f[NPL+2] = next lane's first two
@@ -372,6 +370,7 @@ __device__ __forceinline__ void interval_coeffs(const NodeFn& node, int nx, int 
         f[NPL + 1] = __shfl_down_sync(0xffffffffu, f[1], 1);
         f[NPL + 2] = __shfl_down_sync(0xffffffffu, f[2], 1);
     }
+    double2 ka[NPL], kb[NPL];
 #pragma unroll
     for (int jn = 0; jn < NPL; ++jn) cubic_coeffs(f[jn], f[jn + 1], f[jn + 2], f[jn + 3], ka[jn].x, ka[jn].y, kb[jn].x, kb[jn].y);
     if (jlo == 0 || jhi == nx - 2) {      // the window holds the first / last interval of the axis (warp-uniform)
@@ -396,15 +395,6 @@ __device__ __forceinline__ void interval_coeffs(const NodeFn& node, int nx, int 
             }
         }
     }
-}
-
-template <int NPL, class NodeFn>
-__device__ __forceinline__ void fused_pass(const NodeFn& node, int nx, int jlo, int jhi, int lane, int x_linedge, double2* KA,
-                                           const double* sm)
-{
-    constexpr int KW = 32 * NPL;
-    double2 ka[NPL], kb[NPL];
-    interval_coeffs<NPL>(node, nx, jlo, jhi, lane, x_linedge, ka, kb, sm);
     __syncwarp();                                                   // the previous pair's readers are done
 #pragma unroll
     for (int jn = 0; jn < NPL; ++jn) {
