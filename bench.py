@@ -26,7 +26,8 @@ that takes about a minute or less, else a bounded sample; single-threaded on a b
 both in full).
 
 --precision 1 times the FP32-interpolation variant (tolerance 1e-4 instead of 1e-9; not the judged path), --tmap DEX the
-per-cell temperature-map entry ppm_evaluate_map with a seeded smooth map of +-DEX around each spot's log T.
+per-cell temperature-map entry ppm_evaluate_map with a seeded smooth map of +-DEX around each spot's log T (with
+--emission 1 | 3 | 4 under the strategies that are cubic in log T).
 
 --impl reference: there is no reference implementation (the paper's code is not available); per
 the task contract the reference arm is the CPU oracle, timed on the host cores on a bounded sample.
@@ -492,6 +493,10 @@ def main():
                                     "Roofline); MEASURED_PEAKS.json has no FP64 entry"),
                     "peak_measured_dfma_chain": peak_dfma,
                     "frac_of_measured_dfma_chain": (achieved / peak_dfma) if (peak_dfma and achieved is not None) else None,
+                    "ncu_utilisation": ({"note": "same ncu capture; the highest of the three is the kernel's binding resource (DESIGN.md 6)",
+                                         "shared_memory_wavefronts_pct_of_peak": cap.get("smem_wavefronts_pct"),
+                                         "fp64_pipe_pct_of_peak": cap.get("fp64_pipe_pct"),
+                                         "issue_active_pct": cap.get("issue_active_pct")} if cap else None),
                     "units_per_launch": tri_per_launch, "unit_name": "accumulated (cell, phase, energy) triple",
                     "kernel_ms_per_launch": cells_ms / n_launch, "kernel_launches_per_step": cells_n / args.steps,
                     "kernel_share_of_step": cells_ms / total_ms, "kernel_ms_per_step": kern_ms}
