@@ -493,6 +493,13 @@ def main():
                                     "Roofline); MEASURED_PEAKS.json has no FP64 entry"),
                     "peak_measured_dfma_chain": peak_dfma,
                     "frac_of_measured_dfma_chain": (achieved / peak_dfma) if (peak_dfma and achieved is not None) else None,
+                    # the kernel's binding resource: shared-memory wavefronts of this launch (ncu capture) / the
+                    # kernel's live CUDA-event time, against 1 wavefront (128 B) per clock and SM
+                    "shared_memory": ({"wavefronts_per_launch": cap.get("smem_wavefronts"),
+                                       "achieved_gwavefronts_per_s": cap["smem_wavefronts"] / kern_s / 1e9,
+                                       "peak_gwavefronts_per_s": 148 * 1.965,
+                                       "frac": cap["smem_wavefronts"] / kern_s / (148 * 1.965e9)}
+                                      if (cap and cap.get("smem_wavefronts")) else None),
                     "ncu_utilisation": ({"note": "same ncu capture; the highest of the three is the kernel's binding resource (DESIGN.md 6)",
                                          "shared_memory_wavefronts_pct_of_peak": cap.get("smem_wavefronts_pct"),
                                          "fp64_pipe_pct_of_peak": cap.get("fp64_pipe_pct"),
