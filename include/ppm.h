@@ -51,7 +51,8 @@ extern "C" {
 #define PPM_STATUS_COMPACTNESS 1  /* R_S/R outside (0, 0.56] (reading R4) */
 #define PPM_STATUS_INPUT       2  /* non-finite input, beta_eq >= 1, bad M/R/D/cos i */
 #define PPM_STATUS_SPOT        4  /* invalid spot (zeta <= 0, angles outside [0, pi]) */
-#define PPM_STATUS_MAP_WINDOW  8  /* ppm_evaluate_map under emission 1, 3, 4: a row's logx window exceeds the slice buffers */
+#define PPM_STATUS_MAP_WINDOW  8  /* ppm_evaluate_map under emission 1, 3, 4: a row's logx window exceeds the slice buffers;
+                                     with precision = 1: a log T interval's cells span more than 0.5 dex */
 
 #define PPM_EMISSION_BLACKBODY   0  /* isotropic blackbody, Eq C.5 */
 #define PPM_EMISSION_TABLE_CUBIC 1  /* 4-D table, cubic Lagrange on all axes (strategy a) */
@@ -123,7 +124,9 @@ int ppm_evaluate(ppm_ctx* ctx, const double* params_dev, int B, double* flux_dev
  * phi)"; reading R24): logT_map_dev [B][n_spots][n_theta][n_phi] holds log10 T_eff/K of every cell of every spot's mesh
  * (box grid or HEALPix); a cell emits iff it passes the spot's geometric mask (centre within zeta, outside the omitted
  * cap) AND its entry is finite -- NaN marks a cell that does not emit.  The spots' own log10 T parameters are ignored.
- * Needs table emission, precision = 0 and interp_domain = 0; otherwise PPM_ERR_STATE.  emission =
+ * Needs table emission and interp_domain = 0 (precision = 1, FP32 interpolation, only with emission =
+ * PPM_EMISSION_TABLE_MIXED: k_cells_map32; there an interval whose cells span more than 0.5 dex in log T -- cells far
+ * outside the axis -- gives PPM_STATUS_MAP_WINDOW); otherwise PPM_ERR_STATE.  emission =
  * PPM_EMISSION_TABLE_MIXED (strategy d: linear in log T, two node slices per log T interval) is the fast path; the
  * strategies that are cubic in log T (emission 1, 3, 4) need four node slices per interval, run on a finer energy tiling
  * and cannot hold a row whose cell temperatures lie so far outside the table's log T axis that one interval's logx

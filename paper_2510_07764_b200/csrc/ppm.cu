@@ -21,6 +21,7 @@
 #include "ppm_cells_lin.cuh"
 #include "ppm_cells_map.cuh"
 #include "ppm_cells_map4.cuh"
+#include "ppm_cells_map32.cuh"
 #include "ppm_observe.cuh"
 #include "ppm_chain.cuh"
 
@@ -637,6 +638,32 @@ static int dispatch_cells_map4(ppm_ctx* c, const CellArgs& a, dim3 grid, int thr
     return PPM_OK;
 }
 
+// shared memory of k_cells_map32 (ppm_cells_map32.cuh layout; the tail pad keeps out-of-window node reads inside)
+static size_t cells_map32_smem(const ppm_ctx* c, int nw)
+{
+    return sizeof(double) * ((size_t)nw * (2 * 32 * c->npl + 3 * 64 + 16) + 4 * (size_t)(c->n_fp + 1) + c->nmu + c->nT + 1) +
+           sizeof(float) * (2 * (size_t)c->nmu * c->nx + 32 * c->npl + 32);
+}
+
+template <int EPL>
+static int dispatch_cells_map32(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
+{
+#define PPM_LAUNCH_MAP32(NPLV)                                                                                            \
+    do {                                                                                                                  \
+        CK(cudaFuncSetAttribute(k_cells_map32<EPL, NPLV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+        k_cells_map32<EPL, NPLV><<<grid, threads, smem, c->stream>>>(a, c->d_stars);                                      \
+    } while (0)
+    switch (c->npl) {
+    case 1:  PPM_LAUNCH_MAP32(1); break;
+    case 3:  PPM_LAUNCH_MAP32(3); break;
+    case 5:  PPM_LAUNCH_MAP32(5); break;
+    case 7:  PPM_LAUNCH_MAP32(7); break;
+    default: PPM_LAUNCH_MAP32(9); break;
+    }
+#undef PPM_LAUNCH_MAP32
+    return PPM_OK;
+}
+
 template <int EPL, bool WIN>
 static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
@@ -733,6 +760,23 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
         default: rc = dispatch_cells_map4<10>(c, A, grid, c->m4_nw * 32, sm4); break;
         }
         c->launches += 1;
+    } else if (tmap_dev && g.precision == 1) {
+        // temperature-map mode with FP32 interpolation: two full-width FP32 node slices, 16 warps, one launch
+        A.tmap = tmap_dev; A.values = c->d_values; A.axT = c->d_axT; A.nT = c->nT; A.ng = c->ng;
+        A.map_split = 0; A.uniform_e = 0;
+        const size_t sm32 = cells_map32_smem(c, c->nw);
+        if (sm32 > 227 * 1024) { set_err("temperature-map mode (precision = 1): table and template do not fit in shared memory"); return PPM_ERR_ARG; }
+        dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
+        prof_begin(c, KID_CELLS);
+        switch (c->epl) {
+        case 1:  rc = dispatch_cells_map32<1>(c, A, grid, c->nw * 32, sm32); break;
+        case 2:  rc = dispatch_cells_map32<2>(c, A, grid, c->nw * 32, sm32); break;
+        case 4:  rc = dispatch_cells_map32<4>(c, A, grid, c->nw * 32, sm32); break;
+        case 5:  rc = dispatch_cells_map32<5>(c, A, grid, c->nw * 32, sm32); break;
+        case 8:  rc = dispatch_cells_map32<8>(c, A, grid, c->nw * 32, sm32); break;
+        default: rc = dispatch_cells_map32<10>(c, A, grid, c->nw * 32, sm32); break;
+        }
+        c->launches += 1;
     } else if (tmap_dev) {
         // temperature-map mode: two FP64 log T node slices in shared memory.  Full-width slices leave room for 8 warps;
         // slices cut to the logx columns a row's interval can reach (wst columns) leave room for 16.  Both kernels are
@@ -827,8 +871,10 @@ extern "C" int ppm_evaluate_map(ppm_ctx* c, const double* params_dev, const doub
     if (B == 0) return PPM_OK;
     ARG(params_dev && logT_map_dev && flux_dev, "null pointer");
     if (B > c->cfg.max_batch) { set_err("B = %d exceeds max_batch = %d", B, c->cfg.max_batch); return PPM_ERR_BATCH; }
-    if (c->cfg.emission == PPM_EMISSION_BLACKBODY || c->cfg.precision != 0 || c->cfg.interp_domain != 0) {
-        set_err("temperature maps need table emission (1-4), precision = 0 and interp_domain = 0"); return PPM_ERR_STATE;
+    if (c->cfg.emission == PPM_EMISSION_BLACKBODY || c->cfg.interp_domain != 0 ||
+        (c->cfg.precision != 0 && c->cfg.emission != PPM_EMISSION_TABLE_MIXED)) {
+        set_err("temperature maps need table emission (1-4) and interp_domain = 0; precision = 1 only with emission = 2");
+        return PPM_ERR_STATE;
     }
     if (!c->have_atm) { set_err("table emission requested but no atmosphere loaded"); return PPM_ERR_STATE; }
     if (c->nT > 64) { set_err("temperature maps support at most 64 log T nodes"); return PPM_ERR_STATE; }

@@ -152,6 +152,42 @@ def test_cubic_map_constant_equals_uniform_and_window_status():
     assert st3[1] == 8 and np.all(np.isnan(g3[1]))
 
 
+@pytest.mark.parametrize("mesh", [0, 1])
+def test_fp32_map_matches_oracle(mesh):
+    """precision = 1 (FP32 interpolation and exponential, tolerance 1e-4 per bin: the paper's production precision) with a
+    temperature map: reference exponents per (row, log T interval); smooth seeded maps over many intervals, both meshes."""
+    conf = gen.config_c3(n_cells=36, n_phase=21, n_energy=70)
+    if mesh:
+        nside = 20
+        conf["cfg"] = dict(conf["cfg"], n_theta=4 * nside - 1, n_phi=4 * nside, mesh=1)
+    rng = np.random.default_rng(131 + mesh)
+    tmap = _smooth_map(conf["cfg"], rng)
+    g, st, _ = _gpu_map(conf, tmap[None], make_ctx(conf, precision=1))
+    ref, so = o.evaluate(conf["cfg"], conf["energies"], conf["params"][0], oracle_atm(), tmap=tmap)
+    assert st[0] == 0 and so == 0 and ref.max() > 0
+    assert max_rel_err(g[0], ref) <= 1e-4
+
+
+def test_fp32_map_target_size_edges_and_status():
+    """FP32 maps at the T size (300 energies, clamped upper energies) against the FP64 map kernel (itself at 1e-9 of the
+    oracle); temperatures slightly outside the axis work, an interval spanning more than 0.5 dex gives the status bit."""
+    conf = gen.config_t()
+    cfg = conf["cfg"]
+    tmap = gen.smooth_temperature_map(cfg, conf["params"], 0.3)
+    g64, st64, _ = _gpu_map(conf, tmap)
+    g32, st32, ctx32 = _gpu_map(conf, tmap, make_ctx(conf, precision=1))
+    assert st64[0] == 0 and st32[0] == 0 and max_rel_err(g32[0], g64[0]) <= 1e-4
+    t2 = np.array(tmap, copy=True)
+    t2[0, 0, 100:140, ::3] = 4.85                                                # 0.25 dex below the axis: still inside FP32's range
+    g64b, _, _ = _gpu_map(conf, t2)
+    g32b, st32b, _ = _gpu_map(conf, t2, ctx32)
+    assert st32b[0] == 0 and max_rel_err(g32b[0], g64b[0]) <= 1e-4
+    t3 = np.array(tmap, copy=True)
+    t3[0, 1, 50:60, ::2] = 7.6                                                   # 0.8 dex above the axis
+    g32c, st32c, _ = _gpu_map(conf, t3, ctx32)
+    assert st32c[0] == 8 and np.all(np.isnan(g32c[0]))
+
+
 def test_rows_split_between_the_windowed_and_the_full_width_launch():
     """Temperatures far outside the table's log T axis keep their own kT (reading R13b), which moves the row's logx
     window by tens of columns: such rows do not fit the windowed slice buffers and go to the full-width launch, the
