@@ -248,6 +248,18 @@ __global__ void __launch_bounds__(512, 1) k_cells_map32(CellArgs A, StarD* stars
                             const float y = fmaf(fmaf(fmaf(c4.w, tau, c4.z), tau, c4.y), tau, c4.x) - yoff[i];
                             acc32[i] += ex2_approx(y);
                         }
+                    } else if (q + uef_first >= 0) {
+                        // only the upper energies leave the table (the common clamped case): one-sided clamp
+#pragma unroll
+                        for (int i = 0; i < EPL; ++i) {
+                            long long s = q + uef[i];
+                            s = s > s_top ? s_top : s;                              // clamp to the table (reading R13b)
+                            const int shi = (int)(s >> 32);
+                            const float4 c4 = K4q[shi >> 20];
+                            const float tau = __int_as_float((__funnelshift_l((int)s, shi, 3) & 0x007FFFFF) | 0x3F800000) - 1.5f;
+                            const float y = fmaf(fmaf(fmaf(c4.w, tau, c4.z), tau, c4.y), tau, c4.x) - yoff[i];
+                            acc32[i] += ex2_approx(y);
+                        }
                     } else {
 #pragma unroll
                         for (int i = 0; i < EPL; ++i) {

@@ -15,7 +15,8 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 JSON_PATH = os.path.join(HERE, "ncu_captured.json")
-HASHED = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells32.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh")
+HASHED = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh")
+HASHED_P1 = ("ppm_cells32.cuh", "ppm_cells_map32.cuh")        # added for the keys of precision = 1 (":p1")
 
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
         "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "s": 1.0, "usecond": 1e-6, "nsecond": 1e-9, "msecond": 1e-3, "second": 1.0}
@@ -58,9 +59,9 @@ def _code_only(text):
     return " ".join(text.split())
 
 
-def source_hash():
+def source_hash(precision=0):
     h = hashlib.sha256()
-    for f in HASHED:
+    for f in HASHED + (HASHED_P1 if precision == 1 else ()):
         with open(os.path.join(HERE, "csrc", f), "r") as fh:
             h.update(_code_only(fh.read()).encode())
     return h.hexdigest()[:16]
@@ -101,7 +102,7 @@ def main():
     a = ap.parse_args()
     c = parse(a.raw_csv, a.kernel)
     c["dram_bytes"] = c.get("dram_read_bytes", 0.0) + c.get("dram_write_bytes", 0.0)
-    c["source_hash"] = source_hash()
+    c["source_hash"] = source_hash(1 if ":p1" in a.key else 0)
     c["profile"] = a.profile
     if not a.no_write:
         try:
