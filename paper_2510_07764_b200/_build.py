@@ -1,6 +1,7 @@
 """Build paper_2510_07764_b200/libppm_b200.so (the C-ABI library of include/ppm.h) in-tree with nvcc
 for sm_100a.  `python -m paper_2510_07764_b200._build` or `_build.build()`; rebuilt only when a source
-is newer than the library.  nvcc cross-compiles without a GPU."""
+is newer than the library.  nvcc cross-compiles without a GPU.  The translation units (ppm.cu and the
+cell-kernel launchers launch_*.cu) are compiled in parallel and linked into one shared library."""
 import glob
 import os
 import shutil
@@ -14,7 +15,8 @@ CSRC = os.path.join(_HERE, "csrc")
 BOUNDS = os.environ.get("PPM_BOUNDS", "") not in ("", "0")
 LIB = os.path.join(_HERE, "libppm_b200_bounds.so" if BOUNDS else "libppm_b200.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC"]
+LINK_FLAGS = ["-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"]
 
 
 def sources():
@@ -33,13 +35,32 @@ def build(force: bool = False, verbose: bool = False) -> str:
     srcs = sources()
     if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(s) for s in srcs):
         return LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (["-DPPM_BOUNDS"] if BOUNDS else []) + \
-          ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB + ".tmp", os.path.join(CSRC, "ppm.cu")]
-    res = subprocess.run(cmd, capture_output=True, text=True)
+    nvcc = nvcc_path()
+    units = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    objdir = os.path.join(_HERE, "build", "bounds" if BOUNDS else "obj")
+    os.makedirs(objdir, exist_ok=True)
+    common = NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (["-DPPM_BOUNDS"] if BOUNDS else []) + \
+             ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    procs = []
+    for u in units:
+        obj = os.path.join(objdir, os.path.basename(u)[:-3] + ".o")
+        logf = open(obj + ".log", "w+")                      # a file, not a pipe: no unit ever blocks on a full pipe
+        procs.append((logf, obj, subprocess.Popen([nvcc] + common + ["-c", "-o", obj, u], stdout=logf, stderr=subprocess.STDOUT)))
+    log, failed = "", False
+    for logf, obj, pr in procs:
+        pr.wait()
+        logf.seek(0)
+        log += logf.read()
+        logf.close()
+        failed = failed or pr.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed:\n" + log)
+    res = subprocess.run([nvcc] + LINK_FLAGS + ["-o", LIB + ".tmp"] + [obj for _, obj, _ in procs],
+                         capture_output=True, text=True)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
+        raise RuntimeError("nvcc link failed:\n" + res.stdout + res.stderr)
     if verbose:
-        print(res.stderr)
+        print(log)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

@@ -17,11 +17,8 @@
 #include "ppm_common.cuh"
 #include "ppm_geodesic.cuh"
 #include "ppm_cells.cuh"
-#include "ppm_cells32.cuh"
-#include "ppm_cells_lin.cuh"
-#include "ppm_cells_map.cuh"
-#include "ppm_cells_map4.cuh"
-#include "ppm_cells_map32.cuh"
+#include "ppm_rowops.cuh"
+#include "ppm_launch.h"
 #include "ppm_observe.cuh"
 #include "ppm_chain.cuh"
 
@@ -499,83 +496,22 @@ extern "C" int ppm_set_response(ppm_ctx* c, int n_channel, int band_w, const int
 // ------------------------------------------------------------------------------------------------
 // evaluation
 // ------------------------------------------------------------------------------------------------
-template <typename K>
-static int launch_cells(ppm_ctx* c, K kernel, const CellArgs& a, dim3 grid, int threads, size_t smem)
+static LaunchShape shape_of(const ppm_ctx* c, dim3 grid, int threads, size_t smem, int epl, int npl)
 {
-    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kernel<<<grid, threads, smem, c->stream>>>(a);
-    return PPM_OK;
+    LaunchShape L;
+    L.stream = c->stream; L.grid = grid; L.threads = threads; L.smem = smem; L.epl = epl; L.npl = npl;
+    return L;
 }
 
-template <int EPL>
-static int dispatch_cells_tab32(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_tab32<EPL, 1>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_tab32<EPL, 3>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_tab32<EPL, 5>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_tab32<EPL, 7>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_tab32<EPL, 9>, a, grid, threads, smem);
-    }
-}
-
-template <int EPL>
-static int dispatch_cells_lin(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_lin<EPL, 1>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_lin<EPL, 3>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_lin<EPL, 5>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_lin<EPL, 7>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_lin<EPL, 9>, a, grid, threads, smem);
-    }
-}
-
-template <int EPL>
-static int dispatch_cells_tab(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    if (c->cfg.interp_domain == 1) return dispatch_cells_lin<EPL>(c, a, grid, threads, smem);
-    if (c->cfg.precision == 1) return dispatch_cells_tab32<EPL>(c, a, grid, threads, smem);
-    if constexpr (EPL >= 2) {
-        if (a.uniform_e) {
-            switch (c->npl) {
-            case 1:  return launch_cells(c, k_cells_tab<EPL, 1, true>, a, grid, threads, smem);
-            case 3:  return launch_cells(c, k_cells_tab<EPL, 3, true>, a, grid, threads, smem);
-            case 5:  return launch_cells(c, k_cells_tab<EPL, 5, true>, a, grid, threads, smem);
-            case 7:  return launch_cells(c, k_cells_tab<EPL, 7, true>, a, grid, threads, smem);
-            default: return launch_cells(c, k_cells_tab<EPL, 9, true>, a, grid, threads, smem);
-            }
-        }
-    }
-    switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_tab<EPL, 1, false>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_tab<EPL, 3, false>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_tab<EPL, 5, false>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_tab<EPL, 7, false>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_tab<EPL, 9, false>, a, grid, threads, smem);
-    }
-}
-
+// the uniform-temperature cell kernel of the context's mode (launch_*.cu)
 static int dispatch_cells(ppm_ctx* c, bool table, const CellArgs& a, dim3 grid, int threads, size_t smem)
 {
-    if (table) {
-        switch (c->epl) {
-        case 1:  return dispatch_cells_tab<1>(c, a, grid, threads, smem);
-        case 2:  return dispatch_cells_tab<2>(c, a, grid, threads, smem);
-        case 4:  return dispatch_cells_tab<4>(c, a, grid, threads, smem);
-        case 5:  return dispatch_cells_tab<5>(c, a, grid, threads, smem);
-        case 8:  return dispatch_cells_tab<8>(c, a, grid, threads, smem);
-        default: return dispatch_cells_tab<10>(c, a, grid, threads, smem);
-        }
-    }
-    switch (c->epl) {
-    case 1:  return launch_cells(c, k_cells_bb<1>, a, grid, threads, smem);
-    case 2:  return launch_cells(c, k_cells_bb<2>, a, grid, threads, smem);
-    case 4:  return launch_cells(c, k_cells_bb<4>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_bb<5>, a, grid, threads, smem);
-    case 8:  return launch_cells(c, k_cells_bb<8>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_bb<10>, a, grid, threads, smem);
-    }
+    const LaunchShape L = shape_of(c, grid, threads, smem, c->epl, c->npl);
+    if (!table) CK(launch_cells_bb(L, a));
+    else if (c->cfg.interp_domain == 1) CK(launch_cells_lin(L, a));
+    else if (c->cfg.precision == 1) CK(launch_cells_tab32(L, a));
+    else CK(launch_cells_tab(L, a));
+    return PPM_OK;
 }
 
 // shared memory of k_cells_map with `nw` warps (ppm_cells_map.cuh layout)
@@ -625,19 +561,6 @@ static void choose_map4_tiling(ppm_ctx* c, const std::vector<double>& ue)
     }
 }
 
-template <int EPL>
-static int dispatch_cells_map4(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    if (c->m4_npl == 1) {
-        CK(cudaFuncSetAttribute(k_cells_map4<EPL, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_cells_map4<EPL, 1><<<grid, threads, smem, c->stream>>>(a, c->d_stars);
-    } else {
-        CK(cudaFuncSetAttribute(k_cells_map4<EPL, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_cells_map4<EPL, 3><<<grid, threads, smem, c->stream>>>(a, c->d_stars);
-    }
-    return PPM_OK;
-}
-
 // shared memory of k_cells_map32 (ppm_cells_map32.cuh layout; the tail pad keeps out-of-window node reads inside)
 static size_t cells_map32_smem(const ppm_ctx* c, int nw)
 {
@@ -645,47 +568,6 @@ static size_t cells_map32_smem(const ppm_ctx* c, int nw)
            sizeof(float) * (2 * (size_t)c->nmu * c->nx + 32 * c->npl + 32);
 }
 
-template <int EPL>
-static int dispatch_cells_map32(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-#define PPM_LAUNCH_MAP32(NPLV)                                                                                            \
-    do {                                                                                                                  \
-        CK(cudaFuncSetAttribute(k_cells_map32<EPL, NPLV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
-        k_cells_map32<EPL, NPLV><<<grid, threads, smem, c->stream>>>(a, c->d_stars);                                      \
-    } while (0)
-    switch (c->npl) {
-    case 1:  PPM_LAUNCH_MAP32(1); break;
-    case 3:  PPM_LAUNCH_MAP32(3); break;
-    case 5:  PPM_LAUNCH_MAP32(5); break;
-    case 7:  PPM_LAUNCH_MAP32(7); break;
-    default: PPM_LAUNCH_MAP32(9); break;
-    }
-#undef PPM_LAUNCH_MAP32
-    return PPM_OK;
-}
-
-template <int EPL, bool WIN>
-static int dispatch_cells_map(ppm_ctx* c, const CellArgs& a, dim3 grid, int threads, size_t smem)
-{
-    if constexpr (WIN && EPL >= 4) {                                    // the stepped coordinate (EnergyCoord): windowed kernel only
-        if (a.uniform_e) {
-            switch (c->npl) {
-            case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN, true>, a, grid, threads, smem);
-            case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN, true>, a, grid, threads, smem);
-            case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN, true>, a, grid, threads, smem);
-            case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN, true>, a, grid, threads, smem);
-            default: return launch_cells(c, k_cells_map<EPL, 9, WIN, true>, a, grid, threads, smem);
-            }
-        }
-    }
-    switch (c->npl) {
-    case 1:  return launch_cells(c, k_cells_map<EPL, 1, WIN, false>, a, grid, threads, smem);
-    case 3:  return launch_cells(c, k_cells_map<EPL, 3, WIN, false>, a, grid, threads, smem);
-    case 5:  return launch_cells(c, k_cells_map<EPL, 5, WIN, false>, a, grid, threads, smem);
-    case 7:  return launch_cells(c, k_cells_map<EPL, 7, WIN, false>, a, grid, threads, smem);
-    default: return launch_cells(c, k_cells_map<EPL, 9, WIN, false>, a, grid, threads, smem);
-    }
-}
 
 static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* flux_dev, int32_t* status_dev,
                         const double* tmap_dev = nullptr)
@@ -751,14 +633,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
         dim3 grid(c->nchunk, (g.n_phase + c->m4_nw - 1) / c->m4_nw, nb * c->m4_ntile);
         const size_t sm4 = cells_map4_smem(c, c->m4_nw, c->m4_npl, c->m4_wst);
         prof_begin(c, KID_CELLS);
-        switch (c->m4_epl) {
-        case 1:  rc = dispatch_cells_map4<1>(c, A, grid, c->m4_nw * 32, sm4); break;
-        case 2:  rc = dispatch_cells_map4<2>(c, A, grid, c->m4_nw * 32, sm4); break;
-        case 4:  rc = dispatch_cells_map4<4>(c, A, grid, c->m4_nw * 32, sm4); break;
-        case 5:  rc = dispatch_cells_map4<5>(c, A, grid, c->m4_nw * 32, sm4); break;
-        case 8:  rc = dispatch_cells_map4<8>(c, A, grid, c->m4_nw * 32, sm4); break;
-        default: rc = dispatch_cells_map4<10>(c, A, grid, c->m4_nw * 32, sm4); break;
-        }
+        { const cudaError_t le = launch_cells_map4(shape_of(c, grid, c->m4_nw * 32, sm4, c->m4_epl, c->m4_npl), A, c->d_stars); CK(le); rc = PPM_OK; }
         c->launches += 1;
     } else if (tmap_dev && g.precision == 1) {
         // temperature-map mode with FP32 interpolation: two full-width FP32 node slices, 16 warps, one launch
@@ -768,14 +643,7 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
         if (sm32 > 227 * 1024) { set_err("temperature-map mode (precision = 1): table and template do not fit in shared memory"); return PPM_ERR_ARG; }
         dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
         prof_begin(c, KID_CELLS);
-        switch (c->epl) {
-        case 1:  rc = dispatch_cells_map32<1>(c, A, grid, c->nw * 32, sm32); break;
-        case 2:  rc = dispatch_cells_map32<2>(c, A, grid, c->nw * 32, sm32); break;
-        case 4:  rc = dispatch_cells_map32<4>(c, A, grid, c->nw * 32, sm32); break;
-        case 5:  rc = dispatch_cells_map32<5>(c, A, grid, c->nw * 32, sm32); break;
-        case 8:  rc = dispatch_cells_map32<8>(c, A, grid, c->nw * 32, sm32); break;
-        default: rc = dispatch_cells_map32<10>(c, A, grid, c->nw * 32, sm32); break;
-        }
+        { const cudaError_t le = launch_cells_map32(shape_of(c, grid, c->nw * 32, sm32, c->epl, c->npl), A, c->d_stars); CK(le); rc = PPM_OK; }
         c->launches += 1;
     } else if (tmap_dev) {
         // temperature-map mode: two FP64 log T node slices in shared memory.  Full-width slices leave room for 8 warps;
@@ -801,28 +669,14 @@ static int evaluate_sub(ppm_ctx* c, const double* params_dev, int nb, double* fl
             W.nw = 16;
             dim3 gridw(c->nchunk, (g.n_phase + 15) / 16, nb * c->n_etile);
             const size_t smw = cells_map_smem(c, 16, wst);
-            switch (c->epl) {
-            case 1:  rc = dispatch_cells_map<1, true>(c, W, gridw, 512, smw); break;
-            case 2:  rc = dispatch_cells_map<2, true>(c, W, gridw, 512, smw); break;
-            case 4:  rc = dispatch_cells_map<4, true>(c, W, gridw, 512, smw); break;
-            case 5:  rc = dispatch_cells_map<5, true>(c, W, gridw, 512, smw); break;
-            case 8:  rc = dispatch_cells_map<8, true>(c, W, gridw, 512, smw); break;
-            default: rc = dispatch_cells_map<10, true>(c, W, gridw, 512, smw); break;
-            }
+            { const cudaError_t le = launch_cells_map(shape_of(c, gridw, 512, smw, c->epl, c->npl), W, true); CK(le); rc = PPM_OK; }
             c->launches += 1;
         }
         if (!rc) {
             A.nw = nwm;
             dim3 grid(c->nchunk, (g.n_phase + nwm - 1) / nwm, nb * c->n_etile);
             const size_t smem_map = cells_map_smem(c, nwm, c->nx);
-            switch (c->epl) {
-            case 1:  rc = dispatch_cells_map<1, false>(c, A, grid, nwm * 32, smem_map); break;
-            case 2:  rc = dispatch_cells_map<2, false>(c, A, grid, nwm * 32, smem_map); break;
-            case 4:  rc = dispatch_cells_map<4, false>(c, A, grid, nwm * 32, smem_map); break;
-            case 5:  rc = dispatch_cells_map<5, false>(c, A, grid, nwm * 32, smem_map); break;
-            case 8:  rc = dispatch_cells_map<8, false>(c, A, grid, nwm * 32, smem_map); break;
-            default: rc = dispatch_cells_map<10, false>(c, A, grid, nwm * 32, smem_map); break;
-            }
+            { const cudaError_t le = launch_cells_map(shape_of(c, grid, nwm * 32, smem_map, c->epl, c->npl), A, false); CK(le); rc = PPM_OK; }
         }
     } else {
         dim3 grid(c->nchunk, c->npg, nb * c->n_etile);
