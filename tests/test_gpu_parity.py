@@ -281,8 +281,15 @@ def test_uniform_and_general_energy_paths():
     assert not ctx2.uniform_energy()
     ref2, _ = oracle_flux(lin)
     e_gen = max_rel_err(g2[0], ref2)
-    report("energy_paths", uniform=e_uni, general=e_gen)
-    assert st[0] == 0 and st2[0] == 0 and e_uni <= TOL and e_gen <= TOL
+    # two full energy tiles (640 = 2 x 320 energies) on the stepped coordinate: each tile anchors its own lanes
+    two = gen.config_c2(n_cells=12, n_phase=9, n_energy=640)
+    two["energies"] = gen.logspace(0.1, 15.0, 640)
+    g3, st3, ctx3 = gpu_flux(two)
+    assert ctx3.uniform_energy()
+    ref3, _ = oracle_flux(two)
+    e_two = max_rel_err(g3[0], ref3)
+    report("energy_paths", uniform=e_uni, general=e_gen, two_tiles=e_two)
+    assert st[0] == 0 and st2[0] == 0 and st3[0] == 0 and e_uni <= TOL and e_gen <= TOL and e_two <= TOL
 
 
 def test_narrow_energy_band_uses_a_small_window():
