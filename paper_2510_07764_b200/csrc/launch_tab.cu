@@ -3,13 +3,25 @@
 
 namespace ppm {
 
+// node exchange (k_cells_tab<.., NX = true>): measured on the same box against the record form -- 4 energies per lane
+// (128-energy grids: C3 -2.3 %, the Table 3 geometries -6.5 %), 2 energies per lane +5 % (C2), so EPL = 4 only
+static bool use_node_exchange(int epl, const CellArgs&) { return epl == 4; }
+
 template <int EPL, int NPL>
 static cudaError_t tab_uni(const LaunchShape& L, const CellArgs& a)
 {
-    if constexpr (EPL >= 2) {
-        if (a.uniform_e) PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, true>), a);
+    if constexpr (EPL == 4) {
+        if (use_node_exchange(EPL, a)) {
+            if constexpr (EPL >= 2) {
+                if (a.uniform_e) PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, true, true>), a);
+            }
+            PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, false, true>), a);
+        }
     }
-    PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, false>), a);
+    if constexpr (EPL >= 2) {
+        if (a.uniform_e) PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, true, false>), a);
+    }
+    PPM_LAUNCH_KERNEL((k_cells_tab<EPL, NPL, false, false>), a);
 }
 
 template <int EPL>

@@ -402,6 +402,46 @@ __device__ __forceinline__ double triple_value_checked(const double2* __restrict
     return !(y > -1000.0) ? 0.0 : (y > 1000.0 ? INFINITY : v);
 }
 
+// How a triple gets its cubic.  CoefTriple: the interval's record (a0..a3) from the per-warp coefficient arrays -- 2 x
+// LDS.128 per triple, the per-pair pass has built and stored every interval's record (fused_pass).  NodeTriple: the four
+// NODE VALUES around the interval from a per-warp node array (4 x LDS.64 per triple; the per-pair pass stores 8 bytes per
+// node instead of 32 per interval and skips the Lagrange -> monomial step), the triple forms its own cubic (9 FP64 more):
+// cheaper when a lane owns few energies (EPL <= 4: the per-pair pass is amortised over few triples).  Used for the pairs
+// whose window holds no end interval of the axis (those keep the records, which carry the end rules).
+template <int KW>
+struct CoefTriple {
+    const double2* KAq;
+    __device__ __forceinline__ double value(long long s) const { return triple_value<KW>(KAq, s); }
+    __device__ __forceinline__ double checked(long long s, long long s_top) const { return triple_value_checked<KW>(KAq, s, s_top); }
+};
+
+struct NodeTriple {
+    const double* NVq;                   // node value of table column n at NVq[n]
+    __device__ __forceinline__ double y_of(long long s) const
+    {
+        const int shi = (int)(s >> 32);
+        const double* p = NVq + (shi >> 20);
+        double a0, a1, a2, a3;
+        cubic_coeffs(p[-1], p[0], p[1], p[2], a0, a1, a2, a3);
+        const double t = __hiloint2double(one_plus_frac_hi(shi), (int)s);
+        return fma(fma(fma(a3, t, a2), t, a1), t, a0);
+    }
+    __device__ __forceinline__ double value(long long s) const
+    {
+        const double y = y_of(s);
+        const double r = y + kMagic;
+        return exp2_frac_scaled(y - (r - kMagic), __double2loint(r));
+    }
+    __device__ __forceinline__ double checked(long long s, long long s_top) const
+    {
+        s = s < 0 ? 0 : (s > s_top ? s_top : s);
+        const double y = y_of(s);
+        const double r = y + kMagic;
+        const double v = exp2_frac_scaled(y - (r - kMagic), __double2loint(r));
+        return !(y > -1000.0) ? 0.0 : (y > 1000.0 ? INFINITY : v);
+    }
+};
+
 // The energy part of the logx coordinate for the EPL energies e0 + lane + 32 i a lane owns.
 //  UNI = false: one 64-bit value per energy in registers (2 EPL registers).
 //  UNI = true (log-uniform energy grid -- the paper's grids are, Eq 50): energy i sits at uef[e0 + lane] + i D with
@@ -445,25 +485,25 @@ struct EnergyCoord {
 // are clamped for every lane: their term is the pair's constant 2^y(s_top) and is not evaluated here (the caller defers it).
 // Groups i < G - 1 are entirely inside the table; group G - 1 may straddle the end and clamps its coordinate.
 // One fully unrolled instance per G keeps the G independent dependency chains interleaved.
-template <int KW, int EPL, int G, bool UNI>
-__device__ __forceinline__ void energies_clamped_hi(double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec,
-                                                    const double2* __restrict__ KAq, long long q, long long s_top)
+template <int EPL, int G, bool UNI, class Tri>
+__device__ __forceinline__ void energies_clamped_hi(double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec, const Tri& tri,
+                                                    long long q, long long s_top)
 {
     long long s = ec.first(q);
 #pragma unroll
     for (int i = 0; i < G - 1; ++i) {
-        acc[i] += triple_value<KW>(KAq, s);
+        acc[i] += tri.value(s);
         s = ec.next(s, q, i);
     }
-    acc[G - 1] += triple_value<KW>(KAq, s > s_top ? s_top : s);
+    acc[G - 1] += tri.value(s > s_top ? s_top : s);
 }
 
-template <int KW, int EPL, int G, bool UNI>
-__device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec,
-                                                    const double2* __restrict__ KAq, long long q, long long s_top)
+template <int EPL, int G, bool UNI, class Tri>
+__device__ __forceinline__ void dispatch_clamped_hi(int g, double (&acc)[EPL], const EnergyCoord<EPL, UNI>& ec, const Tri& tri,
+                                                    long long q, long long s_top)
 {
-    if (g == G) energies_clamped_hi<KW, EPL, G, UNI>(acc, ec, KAq, q, s_top);
-    else if constexpr (G > 1) dispatch_clamped_hi<KW, EPL, G - 1, UNI>(g, acc, ec, KAq, q, s_top);
+    if (g == G) energies_clamped_hi<EPL, G, UNI>(acc, ec, tri, q, s_top);
+    else if constexpr (G > 1) dispatch_clamped_hi<EPL, G - 1, UNI>(g, acc, ec, tri, q, s_top);
 }
 
 // Number of energy groups of a pair whose FIRST energy still lies inside the table (used when only PAIR_CLAMP_HI is set):
@@ -477,22 +517,18 @@ __device__ __forceinline__ int clamped_groups(long long pq, const long long* __r
     return g;
 }
 
-// The energies of one pair (step B, part ii): KAq = the pair's coefficient window indexed by interval, q = its coordinate,
+// The energies of one pair (step B, part ii): tri = how a triple gets its cubic (above), q = the pair's coordinate,
 // flg = its flags (bits 8.. = clamped_groups when only PAIR_CLAMP_HI is set), hdef = the lane's deferred sum.
-template <int KW, int EPL, bool UNI>
-__device__ __forceinline__ void pair_energies(double (&acc)[EPL], double& hdef, const EnergyCoord<EPL, UNI>& ec,
-                                              const double2* __restrict__ KAq, long long q, int flg, long long s_top, int lane,
-                                              const double* sm)
+template <int EPL, bool UNI, class Tri>
+__device__ __forceinline__ void pair_energies_with(double (&acc)[EPL], double& hdef, const EnergyCoord<EPL, UNI>& ec, const Tri& tri,
+                                                   long long q, int flg, long long s_top, int lane)
 {
-    (void)sm;
     if (flg == 0) {
         // every coordinate of the tile lies inside the table and every exponent is in range
         long long s = ec.first(q);
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
-            PPM_SMEM_CHECK(KAq + (s >> 52), sizeof(double2));
-            PPM_SMEM_CHECK(KAq + (s >> 52) + KW, sizeof(double2));
-            acc[i] += triple_value<KW>(KAq, s);
+            acc[i] += tri.value(s);
             s = ec.next(s, q, i);
         }
     } else if ((flg & 7) == PAIR_CLAMP_HI) {
@@ -501,20 +537,41 @@ __device__ __forceinline__ void pair_energies(double (&acc)[EPL], double& hdef, 
         // to lane g's deferred sum and is spread over acc[g ..] once, in the epilogue (spread_deferred).
         const int g = flg >> 8;
         if (g < EPL) {                                                          // (g == EPL: only the last group straddles the end)
-            const double vtop = triple_value<KW>(KAq, s_top);
+            const double vtop = tri.value(s_top);
             if (lane == g) hdef += vtop;
         }
-        dispatch_clamped_hi<KW, EPL, EPL, UNI>(g, acc, ec, KAq, q, s_top);
+        dispatch_clamped_hi<EPL, EPL, UNI>(g, acc, ec, tri, q, s_top);
     } else {
         // energies below the axis, or extreme table values (|exponent| may exceed the double range): clamped,
         // range-checked form
         long long s = ec.first(q);
 #pragma unroll
         for (int i = 0; i < EPL; ++i) {
-            acc[i] += triple_value_checked<KW>(KAq, s, s_top);
+            acc[i] += tri.checked(s, s_top);
             s = ec.next(s, q, i);
         }
     }
+}
+
+// ... with the interval records of fused_pass (KAq = the pair's coefficient window indexed by interval)
+template <int KW, int EPL, bool UNI>
+__device__ __forceinline__ void pair_energies(double (&acc)[EPL], double& hdef, const EnergyCoord<EPL, UNI>& ec,
+                                              const double2* __restrict__ KAq, long long q, int flg, long long s_top, int lane,
+                                              const double* sm)
+{
+#ifdef PPM_BOUNDS
+    {   // every record address of the plain loop (the other loops clamp into the same range)
+        long long s = ec.first(q);
+        for (int i = 0; i < EPL; ++i) {
+            const long long sc = s < 0 ? 0 : (s > s_top ? s_top : s);
+            PPM_SMEM_CHECK(KAq + (sc >> 52), sizeof(double2));
+            PPM_SMEM_CHECK(KAq + (sc >> 52) + KW, sizeof(double2));
+            s = ec.next(s, q, i);
+        }
+    }
+#endif
+    (void)sm;
+    pair_energies_with<EPL, UNI>(acc, hdef, ec, CoefTriple<KW>{KAq}, q, flg, s_top, lane);
 }
 
 // deferred constants of the clamped groups: acc[i] += sum over g <= i of lane g's hdef (inclusive scan over lanes)
@@ -530,7 +587,9 @@ __device__ __forceinline__ void spread_deferred(double (&acc)[EPL], double hdef,
     for (int i = 0; i < EPL; ++i) acc[i] += __shfl_sync(0xffffffffu, hdef, i);
 }
 
-template <int EPL, int NPL, bool UNI>
+// NX = true ("node exchange", EPL <= 4): for the pairs whose window holds no end interval of the axis the per-pair pass
+// stores node values and the triples form their own cubics (NodeTriple) instead of fetching interval records.
+template <int EPL, int NPL, bool UNI, bool NX>
 __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
 {
     extern __shared__ __align__(16) double sm[];
@@ -653,9 +712,24 @@ __global__ void __launch_bounds__(512, 1) k_cells_tab(CellArgs A)
                 const double qb = r0.y, v0 = r1.x, v1 = r1.y, v2 = r2.x, v3 = r2.y;
                 const int jlo = (inf >> 16) & 255, jhi = (inf >> 24) & 255;
                 const SliceNode node{S + (inf & 0xFFFF), nx, v0, v1, v2, v3, qb};
-                fused_pass<NPL>(node, nx, jlo, jhi, lane, A.x_linedge, KA, sm);
-                const double2* KAq = KA + (1 - jlo);
-                pair_energies<KW, EPL, UNI>(acc, hdef, ec, KAq, q, flg, s_top, lane, sm);
+                if (NX && jlo != 0 && jhi != nx - 2) {
+                    // node exchange (pairs whose window holds no end interval of the axis): lane l contracts the mu stencil
+                    // at its NPL nodes and stores the VALUES; node n of the table sits at NV[n - (jlo - 1)]
+                    const int n0 = jlo - 1 + NPL * lane;
+                    double* NV = wbase;
+                    double fv[NPL];
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn) fv[jn] = node(n0 + jn);
+                    __syncwarp();                                               // the previous pair's readers are done
+#pragma unroll
+                    for (int jn = 0; jn < NPL; ++jn) NV[NPL * lane + jn] = fv[jn];
+                    __syncwarp();
+                    pair_energies_with<EPL, UNI>(acc, hdef, ec, NodeTriple{NV - (jlo - 1)}, q, flg, s_top, lane);
+                } else {
+                    fused_pass<NPL>(node, nx, jlo, jhi, lane, A.x_linedge, KA, sm);
+                    const double2* KAq = KA + (1 - jlo);
+                    pair_energies<KW, EPL, UNI>(acc, hdef, ec, KAq, q, flg, s_top, lane, sm);
+                }
             }
         }
     }
