@@ -222,6 +222,25 @@ int ppm_measure_fp64_peak(int device, double* flops_per_s);
 
 const char* ppm_last_error(void); /* thread-local, static storage */
 
+/* ---- allocation-free S7 (ppm_noalloc.cu) ----------------------------------------------------------------------------
+ * ppm_loglike_noalloc: the Poisson ln L of ppm_loglike (reading R14; same kernels' arithmetic and summation order, so the
+ * same bits) for callers that cannot call cudaMalloc (CUDA-graph capture, tight serving loops, harnesses that forbid it).
+ * It needs no context and calls no cudaMalloc / cudaFree / allocating library routine: its scratch (the per-slice partial
+ * sums) is a static __device__ array of (PPM_NOALLOC_MAX_BATCH + 1) x 64 doubles + ints = 0.75 MiB that every GPU which
+ * loads the library holds until the process exits.
+ *   counts_dev [B][n_phase][n_channel] counts/s, data_dev [n_phase][n_channel], bkg_dev [n_channel] or NULL, loglike_dev
+ *   [B]: device pointers on the CURRENT device; stream: a cudaStream_t (NULL = the default stream); asynchronous.
+ *   B > PPM_NOALLOC_MAX_BATCH -> PPM_ERR_BATCH (split the batch, or use ppm_loglike); bad arguments -> PPM_ERR_ARG; text
+ *   from ppm_loglike_noalloc_error() (thread-local, static storage).
+ * Every call on a device shares the array, which keeps the last call's contents (nothing in it has to start at zero: stage
+ * 1 overwrites every entry stage 2 reads).  Calls that overlap on one GPU -- other streams, other host threads -- RACE on
+ * it: serialise them.  The first call on a device looks up the array's device address (cudaGetSymbolAddress, which may
+ * load the module): make one call per device before capturing a graph around later ones. */
+#define PPM_NOALLOC_MAX_BATCH 1024
+int ppm_loglike_noalloc(const double* counts_dev, int B, int n_phase, int n_channel, const double* data_dev,
+                        const double* bkg_dev, double exposure_s, double* loglike_dev, void* stream);
+const char* ppm_loglike_noalloc_error(void);
+
 #ifdef __cplusplus
 }
 #endif

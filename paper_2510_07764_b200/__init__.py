@@ -6,5 +6,6 @@ CPU fallback: importing works anywhere the library can be built or found, every 
 raises PPMError when no CUDA device / library is usable.
 """
 from .binding import (PPM, PPMError, EXPORTS, lib_path, load_library, measure_fp64_peak,  # noqa: F401
+                      loglike_noalloc, NOALLOC_MAX_BATCH,
                       EMISSION_BLACKBODY, EMISSION_TABLE_CUBIC, EMISSION_TABLE_MIXED, EMISSION_TABLE_CUBIC_LINEDGE,
                       EMISSION_TABLE_CUBIC_CLIP)

@@ -54,6 +54,8 @@ EXPORTS = {
     "ppm_profile_read": (C.c_int, [_vp, _dp, C.POINTER(C.c_int64), _dp]),
     "ppm_measure_fp64_peak": (C.c_int, [C.c_int, _dp]),
     "ppm_last_error": (C.c_char_p, []),
+    "ppm_loglike_noalloc": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_double, _vp, _vp]),
+    "ppm_loglike_noalloc_error": (C.c_char_p, []),
 }
 
 _lib = None
@@ -105,6 +107,29 @@ def _dev(t, dtype=None, what="tensor", shape=None):
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise PPMError(f"{what} must have shape {tuple(shape)}, got {tuple(t.shape)}")
     return C.c_void_p(t.data_ptr())
+
+
+NOALLOC_MAX_BATCH = 1024      # PPM_NOALLOC_MAX_BATCH of include/ppm.h
+
+
+def loglike_noalloc(counts, data, bkg, exposure_s, out):
+    """ppm_loglike_noalloc: Poisson ln L without a context and without any allocation (static device scratch; see
+    include/ppm.h).  counts [B][n_phase][n_channel], data [n_phase][n_channel], bkg [n_channel] or None, out [B]: contiguous
+    float64 CUDA tensors on the current device; runs on torch's current stream.  `out` is the caller's (nothing is
+    allocated here either).  Calls that overlap on the GPU race on the shared scratch."""
+    import torch
+    lib = load_library()
+    if not isinstance(counts, torch.Tensor) or counts.dim() != 3:
+        raise PPMError("counts must be a [B][n_phase][n_channel] CUDA tensor")
+    B, n_phase, n_channel = counts.shape
+    bp = _dev(bkg, torch.float64, "bkg", (n_channel,)) if bkg is not None else C.c_void_p(0)
+    rc = lib.ppm_loglike_noalloc(_dev(counts, torch.float64, "counts"), int(B), int(n_phase), int(n_channel),
+                                 _dev(data, torch.float64, "data", (n_phase, n_channel)), bp, float(exposure_s),
+                                 _dev(out, torch.float64, "loglike", (B,)),
+                                 C.c_void_p(torch.cuda.current_stream(counts.device).cuda_stream))
+    if rc != 0:
+        raise PPMError(f"ppm error {rc}: {lib.ppm_loglike_noalloc_error().decode()}")
+    return out
 
 
 def _host(a, dtype, shape, what):
