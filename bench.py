@@ -216,22 +216,33 @@ def _code_only(text):
     return " ".join(text.split())
 
 
-def kernel_source_hash(precision=0):
-    """sha256 (first 16 hex digits) of the sources that define the cell kernels of this precision: a capture in
-    ncu_captured.json is used only for the kernel build it was taken from."""
+def kernel_source_files(precision=0, tmap=False, domain=0):
+    """the sources that define the cell kernel a bench configuration runs (shared code + that family's file)"""
+    files = ["ppm_common.cuh", "ppm_cells.cuh"]
+    if domain == 1:
+        files.append("ppm_cells_lin.cuh")
+    if tmap:
+        files.append("ppm_cells_map.cuh")
+    if precision == 1:
+        files.append("ppm_cells32.cuh")
+        if tmap:
+            files.append("ppm_cells_map32.cuh")
+    return files
+
+
+def kernel_source_hash(precision=0, tmap=False, domain=0):
+    """sha256 (first 16 hex digits) of the sources that define the cell kernel of this configuration, comments and white
+    space excluded: a capture in ncu_captured.json is used only for the kernel source it was taken from."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2510_07764_b200", "csrc")
-    files = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh")
-    if precision == 1:
-        files += ("ppm_cells32.cuh", "ppm_cells_map32.cuh")
-    for f in files:
+    for f in kernel_source_files(precision, tmap, domain):
         with open(os.path.join(d, f), "r") as fh:
             h.update(_code_only(fh.read()).encode())
     return h.hexdigest()[:16]
 
 
-def ncu_capture_for(key, precision=0):
+def ncu_capture_for(key, precision=0, tmap=False, domain=0):
     """Counters of the `ncu --set full` capture of the cell kernel on exactly this workload key and kernel source, or None."""
     path = os.path.join(ROOT, "paper_2510_07764_b200", "ncu_captured.json")
     try:
@@ -239,7 +250,7 @@ def ncu_capture_for(key, precision=0):
             cap = json.load(f).get("captures", {}).get(key)
     except (OSError, ValueError):
         return None
-    if not cap or cap.get("source_hash") != kernel_source_hash(precision):
+    if not cap or cap.get("source_hash") != kernel_source_hash(precision, tmap, domain):
         return None
     return cap
 
@@ -469,7 +480,7 @@ def main():
         key = "%s:%d:p%d%s" % (args.workload, B, args.precision, "" if args.tmap is None else ":tmap%g" % args.tmap)
         if args.emission is not None or args.interp_domain or args.phase_interp == 3:
             key += ":e%s:d%d:ph%d" % (args.emission, args.interp_domain, args.phase_interp)
-        cap = ncu_capture_for(key, args.precision)
+        cap = ncu_capture_for(key, args.precision, args.tmap is not None, args.interp_domain)
         # precision = 1 runs the per-triple work on the FP32 pipe: 128 FFMA lanes per SM, twice the FP64 figure
         peak_nominal = FP64_NOMINAL_TFLOPS * (2.0 if args.precision == 1 else 1.0)
         achieved = exec_per_unit = traffic = None
@@ -487,7 +498,7 @@ def main():
                     "basis": ("executed FP64 flop per launch (2 DFMA + DADD + DMUL thread instructions, ncu capture of this "
                               "workload and kernel source: %s) / the kernel's CUDA-event time" % cap.get("profile", "?"))
                              if cap else "no ncu capture matches this workload key and kernel source: see algorithmic_*",
-                    "capture_key": key, "kernel_source_hash": kernel_source_hash(args.precision),
+                    "capture_key": key, "kernel_source_hash": kernel_source_hash(args.precision, args.tmap is not None, args.interp_domain),
                     "executed_flop_per_unit": exec_per_unit,
                     "algorithmic_flop_per_unit": FLOP_PER_TRIPLE, "algorithmic_achieved": algorithmic,
                     "algorithmic_frac": algorithmic / peak_nominal,

@@ -210,11 +210,27 @@ __global__ void __launch_bounds__(WIN ? 512 : 256, 1) k_cells_map(CellArgs A)
                 double* dst = buf ? Sb1 : Sb0;
                 const double* src = A.values + ((size_t)node * A.ng + row.bg + go) * gplane + n_lo;
                 const int wcols = n_hi - n_lo + 1;
-                // 128 consecutive threads walk the columns of one mu row (coalesced), blockDim / 128 rows per pass
-                for (int mu_i = threadIdx.x >> 7; mu_i < A.nmu; mu_i += blockDim.x >> 7) {
-                    const double* s0 = src + (size_t)mu_i * nx;
-                    for (int col = threadIdx.x & 127; col < wcols; col += 128)
-                        dst[mu_i * wst + col] = fma(wgb, __ldg(s0 + gplane + col), wga * __ldg(s0 + col));
+                // 128 consecutive threads walk the columns of one mu row (coalesced), blockDim / 128 rows per pass; kDepth
+                // passes' loads are issued before their blends (2 kDepth independent L2 loads in flight per thread: the
+                // staging is latency-bound, and with one pass at a time it cost as much as the interval's arithmetic)
+                constexpr int kDepth = 6;
+                const int rstep = (int)(blockDim.x >> 7);
+                for (int col = threadIdx.x & 127; col < wcols; col += 128) {
+                    for (int mu_0 = threadIdx.x >> 7; mu_0 < A.nmu; mu_0 += kDepth * rstep) {
+                        double va[kDepth], vb[kDepth];
+#pragma unroll
+                        for (int u = 0; u < kDepth; ++u) {
+                            const int mu_i = imin_(mu_0 + u * rstep, A.nmu - 1);
+                            const double* s0 = src + (size_t)mu_i * nx + col;
+                            va[u] = __ldg(s0);
+                            vb[u] = __ldg(s0 + gplane);
+                        }
+#pragma unroll
+                        for (int u = 0; u < kDepth; ++u) {
+                            const int mu_i = mu_0 + u * rstep;
+                            if (mu_i < A.nmu) dst[mu_i * wst + col] = fma(wgb, vb[u], wga * va[u]);
+                        }
+                    }
                 }
             }
             __syncthreads();

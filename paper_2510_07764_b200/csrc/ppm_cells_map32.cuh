@@ -133,8 +133,22 @@ __global__ void __launch_bounds__(512, 1) k_cells_map32(CellArgs A, StarD* stars
                 if (buf) node1 = node; else node0 = node;
                 float* dst = buf ? Sb1 : Sb0;
                 const double* src = A.values + ((size_t)node * A.ng + row.bg + go) * gplane;
-                for (int i = threadIdx.x; i < plane; i += blockDim.x)
-                    dst[i] = (float)fma(wgb, __ldg(src + gplane + i), wga * __ldg(src + i));
+                // kDepth passes' loads are issued before their blends (the staging is bound by L2 latency)
+                constexpr int kDepth = 6;
+                for (int i0 = threadIdx.x; i0 < plane; i0 += kDepth * blockDim.x) {
+                    double va[kDepth], vb[kDepth];
+#pragma unroll
+                    for (int u = 0; u < kDepth; ++u) {
+                        const int i = imin_(i0 + u * (int)blockDim.x, plane - 1);
+                        va[u] = __ldg(src + i);
+                        vb[u] = __ldg(src + gplane + i);
+                    }
+#pragma unroll
+                    for (int u = 0; u < kDepth; ++u) {
+                        const int i = i0 + u * (int)blockDim.x;
+                        if (i < plane) dst[i] = (float)fma(wgb, vb[u], wga * va[u]);
+                    }
+                }
             }
             __syncthreads();
             if (!kvalid) continue;

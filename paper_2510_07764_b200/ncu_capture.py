@@ -15,8 +15,19 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 JSON_PATH = os.path.join(HERE, "ncu_captured.json")
-HASHED = ("ppm_common.cuh", "ppm_cells.cuh", "ppm_cells_map.cuh", "ppm_cells_lin.cuh")
-HASHED_P1 = ("ppm_cells32.cuh", "ppm_cells_map32.cuh")        # added for the keys of precision = 1 (":p1")
+def hashed_files(key):
+    """the sources that define the cell kernel of a capture key (same rule as bench.kernel_source_files)"""
+    files = ["ppm_common.cuh", "ppm_cells.cuh"]
+    if ":d1" in key:
+        files.append("ppm_cells_lin.cuh")
+    if ":tmap" in key:
+        files.append("ppm_cells_map.cuh")
+    if ":p1" in key:
+        files.append("ppm_cells32.cuh")
+        if ":tmap" in key:
+            files.append("ppm_cells_map32.cuh")
+    return files
+
 
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
         "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "s": 1.0, "usecond": 1e-6, "nsecond": 1e-9, "msecond": 1e-3, "second": 1.0}
@@ -59,9 +70,9 @@ def _code_only(text):
     return " ".join(text.split())
 
 
-def source_hash(precision=0):
+def source_hash(key):
     h = hashlib.sha256()
-    for f in HASHED + (HASHED_P1 if precision == 1 else ()):
+    for f in hashed_files(key):
         with open(os.path.join(HERE, "csrc", f), "r") as fh:
             h.update(_code_only(fh.read()).encode())
     return h.hexdigest()[:16]
@@ -102,13 +113,14 @@ def main():
     a = ap.parse_args()
     c = parse(a.raw_csv, a.kernel)
     c["dram_bytes"] = c.get("dram_read_bytes", 0.0) + c.get("dram_write_bytes", 0.0)
-    c["source_hash"] = source_hash(1 if ":p1" in a.key else 0)
+    c["source_hash"] = source_hash(a.key)
+    c["hashed_sources"] = hashed_files(a.key)
     c["profile"] = a.profile
     if not a.no_write:
         try:
             data = json.load(open(JSON_PATH))
         except (OSError, ValueError):
-            data = {"hashed_sources": list(HASHED), "captures": {}}
+            data = {"captures": {}}
         data["captures"][a.key] = c
         with open(JSON_PATH, "w") as f:
             json.dump(data, f, indent=1, sort_keys=True)
