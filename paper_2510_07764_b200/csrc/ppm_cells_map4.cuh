@@ -178,14 +178,32 @@ __global__ void __launch_bounds__(512, 1) k_cells_map4(CellArgs A, StarD* stars_
                 double* dst = Sb + (size_t)bq * plane;
                 const double* src = A.values + ((size_t)node * A.ng + row.bg) * gplane + n_lo;
                 const int wcols = n_hi - n_lo + 1;
-                for (int mu_i = threadIdx.x >> 7; mu_i < A.nmu; mu_i += blockDim.x >> 7) {
-                    const double* s0 = src + (size_t)mu_i * nx;
-                    for (int col = threadIdx.x & 127; col < wcols; col += 128) {
-                        double v = 0.0;
+                // three (mu row, column) passes' loads -- up to 12 independent L2 loads per thread -- are issued before their
+                // blends: the staging is bound by L2 latency (see k_cells_map)
+                constexpr int kDepth = 3;
+                const int rstep = (int)(blockDim.x >> 7);
+                const double wg0 = row.wg[0], wg1 = row.wg[1], wg2 = row.wg[2], wg3 = row.wg[3];
+                for (int col = threadIdx.x & 127; col < wcols; col += 128) {
+                    for (int mu_0 = threadIdx.x >> 7; mu_0 < A.nmu; mu_0 += kDepth * rstep) {
+                        double x[kDepth][4];
 #pragma unroll
-                        for (int gq = 0; gq < 4; ++gq)
-                            if (row.wg[gq] != 0.0) v = fma(row.wg[gq], __ldg(s0 + (size_t)gq * gplane + col), v);
-                        dst[mu_i * wst + col] = v;
+                        for (int u = 0; u < kDepth; ++u) {
+                            const double* s0 = src + (size_t)imin_(mu_0 + u * rstep, A.nmu - 1) * nx + col;
+                            x[u][0] = (wg0 != 0.0) ? __ldg(s0) : 0.0;
+                            x[u][1] = (wg1 != 0.0) ? __ldg(s0 + gplane) : 0.0;
+                            x[u][2] = (wg2 != 0.0) ? __ldg(s0 + 2 * gplane) : 0.0;
+                            x[u][3] = (wg3 != 0.0) ? __ldg(s0 + 3 * gplane) : 0.0;
+                        }
+#pragma unroll
+                        for (int u = 0; u < kDepth; ++u) {
+                            const int mu_i = mu_0 + u * rstep;
+                            double v = 0.0;                                      // zero weights are skipped, as in k_slice
+                            if (wg0 != 0.0) v = fma(wg0, x[u][0], v);
+                            if (wg1 != 0.0) v = fma(wg1, x[u][1], v);
+                            if (wg2 != 0.0) v = fma(wg2, x[u][2], v);
+                            if (wg3 != 0.0) v = fma(wg3, x[u][3], v);
+                            if (mu_i < A.nmu) dst[mu_i * wst + col] = v;
+                        }
                     }
                 }
             }
